@@ -1,0 +1,455 @@
+"""Pins of the CPU oracle against things that are NOT the oracle (CPU only, -m "not gpu").
+
+The paper prints no worked numeric example, so every pin is a closed form, an
+invariant, an exact-rational / library re-computation or brute force on tiny inputs, chosen so that
+a dropped term, a wrong sign, a shifted stencil or a transposed index fails at least one of them.
+Cited passages are lines of /root/reference/PAPER.md.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+from scipy.interpolate import BarycentricInterpolator
+
+import oracle
+from oracle import Grid
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+QS = (2, 4, 6, 8, 10, 12)
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers that do not use the oracle
+# ------------------------------------------------------------------------------------------------
+def exact_weights(q: int, theta: Fraction):
+    """Unique w with sum_m m^p w_m = theta^p, p=0..q-1 (exactness on polynomials of degree < q --
+    the defining property of the interpolant of eq (7)), by Gauss-Jordan in rationals."""
+    ms = [Fraction(m) for m in range(-q // 2 + 1, q // 2 + 1)]
+    A = [[m ** p for m in ms] + [theta ** p] for p in range(q)]
+    for c in range(q):
+        piv = next(r for r in range(c, q) if A[r][c] != 0)
+        A[c], A[piv] = A[piv], A[c]
+        A[c] = [v / A[c][c] for v in A[c]]
+        for r in range(q):
+            if r != c and A[r][c] != 0:
+                A[r] = [vr - A[r][c] * vc for vr, vc in zip(A[r], A[c])]
+    return [A[r][q] for r in range(q)]
+
+
+def small_grid(n, Lx=4 * math.pi, vmax=6.0):
+    lo = [0.0, 0.0, 0.0, -vmax, -vmax, -vmax]
+    dx = [Lx / n[d] for d in range(3)] + [2 * vmax / n[d] for d in range(3, 6)]
+    return Grid(tuple(n), tuple(lo), tuple(dx))
+
+
+def scipy_pencil(g, alpha, q, periodic):
+    """out[j] = value at j+alpha of the degree q-1 polynomial through the q nodes nearest the foot
+    (eq (7): stencil centred on the foot), built by scipy's barycentric Lagrange routine."""
+    n = len(g)
+    k = math.floor(alpha)
+    out = np.empty(n)
+    for j in range(n):
+        idx = np.arange(j + k - q // 2 + 1, j + k + q // 2 + 1)
+        if periodic:
+            vals = g[idx % n]
+        else:
+            vals = np.where((idx >= 0) & (idx < n), g[np.clip(idx, 0, n - 1)], 0.0)
+        out[j] = float(BarycentricInterpolator(idx.astype(float), vals)(j + alpha))
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
+# weights (eq (7))
+# ------------------------------------------------------------------------------------------------
+def test_weights_golden_midpoint_bit_exact():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "lagrange_midpoint.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 7
+    for r in rows:
+        q, (tn, td), den = int(r[0]), map(int, r[1].split("/")), int(r[2])
+        nums = np.array([int(v) for v in r[3:]], dtype=np.float64)
+        assert len(nums) == q
+        w = oracle.lagrange_weights(q, tn / td)
+        assert np.array_equal(w, nums / den), (q, w * den)
+
+
+@pytest.mark.parametrize("q", QS)
+def test_weights_match_exact_rational_moment_solve(q):
+    rng = np.random.default_rng(q)
+    thetas = [0.0, 1.0, 0.5, 0.25, 0.7, 1e-9, 1 - 1e-9] + list(rng.random(6))
+    for th in thetas:
+        w = oracle.lagrange_weights(q, th)
+        we = np.array([float(v) for v in exact_weights(q, Fraction(th))])
+        assert np.max(np.abs(w - we)) <= 4e-16 * np.max(np.abs(we)) * q, (q, th)
+        # the golden file itself, re-derived exactly
+    for r in (Fraction(1, 2), Fraction(1, 4)):
+        we = exact_weights(q, r)
+        assert np.array_equal(oracle.lagrange_weights(q, float(r)), np.array([float(v) for v in we]))
+
+
+@pytest.mark.parametrize("q", QS)
+def test_weights_unit_vectors_symmetry_partition(q):
+    w0, w1 = oracle.lagrange_weights(q, 0.0), oracle.lagrange_weights(q, 1.0)
+    e0 = np.zeros(q); e0[q // 2 - 1] = 1.0          # node m = 0
+    e1 = np.zeros(q); e1[q // 2] = 1.0              # node m = 1
+    assert np.array_equal(np.abs(w0), e0) and np.array_equal(np.abs(w1), e1)   # exactly 0/1 (signed zeros allowed)
+    for th in (0.1, 0.37, 0.5, 0.93):
+        w = oracle.lagrange_weights(q, th)
+        assert abs(w.sum() - 1.0) < 1e-14
+        assert np.allclose(w, oracle.lagrange_weights(q, 1.0 - th)[::-1], rtol=0, atol=1e-15)   # w_m(th)=w_{1-m}(1-th)
+    if q == 2:
+        assert np.array_equal(oracle.lagrange_weights(2, 0.3), np.array([1 - 0.3, 0.3]))
+
+
+# ------------------------------------------------------------------------------------------------
+# property 1: integer-cell shifts are exact permutations (north_star; reading S10)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim", range(6))
+@pytest.mark.parametrize("cells", [1, -1, 3, -11, 0, 19])
+def test_integer_shift_is_permutation(dim, cells):
+    n = [8, 9, 10, 8, 9, 10]
+    rng = np.random.default_rng(dim * 100 + cells + 50)
+    f = rng.random(n)
+    src = np.array([1.0])
+    out = oracle.sweep(f, dim, src, 0, float(cells), 8)     # alpha = -cells  ->  out[j] = f[j - cells]
+    if dim < 3:
+        ref = np.roll(f, cells, axis=dim)
+    else:
+        ref = np.zeros_like(f)
+        nd = n[dim]
+        if abs(cells) < nd:
+            sl_dst = [slice(None)] * 6; sl_src = [slice(None)] * 6
+            if cells >= 0:
+                sl_dst[dim] = slice(cells, nd); sl_src[dim] = slice(0, nd - cells)
+            else:
+                sl_dst[dim] = slice(0, nd + cells); sl_src[dim] = slice(-cells, nd)
+            ref[tuple(sl_dst)] = f[tuple(sl_src)]
+    assert np.array_equal(out, ref)
+
+
+def test_integer_shift_v_dependent_C1():
+    """Reading S10(ii): 8^6, dt = 2*dx1 -> alpha = -2*v_j, v_j = -6+1.5j -> k in {12,9,...,-9}, periodic on n=8."""
+    g = small_grid([8] * 6)
+    rng = np.random.default_rng(7)
+    f = rng.random(g.n)
+    dt = 2.0 * g.dx[0]
+    out = oracle.advect(g, 7, f, 0, None, dt)
+    v = g.nodes(3)
+    assert np.array_equal(v, -6.0 + 1.5 * np.arange(8))
+    for j1 in range(8):
+        cells = int(round(2.0 * v[j1]))                   # out[i] = f[i - cells]
+        assert np.array_equal(out[:, :, :, j1], np.roll(f[:, :, :, j1], cells, axis=0))
+
+
+# ------------------------------------------------------------------------------------------------
+# property 2: polynomials up to the stencil degree are reproduced
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("q", (4, 6, 8, 10))
+@pytest.mark.parametrize("alpha", (0.3, -0.45, 1.7, -2.25))
+def test_polynomial_reproduction(q, alpha):
+    n = 40
+    rng = np.random.default_rng(q)
+    coef = rng.standard_normal(q)                       # degree q-1
+    P = lambda x: np.polyval(coef, (x - 20.0) / 10.0)
+    g = P(np.arange(n, dtype=float))[None, :]
+    out = oracle.sweep_pencils(g, np.array([1.0]), -alpha, q, periodic=False)[0]
+    k = math.floor(alpha)
+    j = np.arange(n)
+    inside = (j + k - q // 2 + 1 >= 0) & (j + k + q // 2 <= n - 1)
+    assert inside.sum() >= n - q - 4
+    err = np.max(np.abs(out[inside] - P(j[inside] + alpha)))
+    assert err < 2e-13 * np.max(np.abs(g)), err
+    # one degree higher is NOT reproduced (the stencil really has q points, not more)
+    g2 = (np.arange(n, dtype=float) - 20.0)[None, :] ** q
+    out2 = oracle.sweep_pencils(g2, np.array([1.0]), -alpha, q, periodic=False)[0]
+    assert np.max(np.abs(out2[inside] - (j[inside] + alpha - 20.0) ** q)) > 1e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# property 3: total mass conserved under periodic constant shifts
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("q", (6, 8, 10))
+def test_mass_conservation_periodic(q):
+    rng = np.random.default_rng(q)
+    g = rng.random((64, 32))
+    for alpha in (0.37, -0.81, 3.3, -17.6):
+        out = oracle.sweep_pencils(g, np.ones(64), -alpha, q, periodic=True)
+        assert abs(out.sum() - g.sum()) < 1e-13 * np.abs(g).sum()
+        assert np.max(np.abs(out.sum(axis=1) - g.sum(axis=1))) < 1e-13 * np.abs(g).sum(axis=1).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# whole-pencil check against scipy's barycentric Lagrange routine and against exact rationals
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("q", (4, 6, 8, 10))
+@pytest.mark.parametrize("periodic", (True, False))
+def test_pencil_against_scipy_barycentric(q, periodic):
+    rng = np.random.default_rng(q + 10 * periodic)
+    n = 13
+    for alpha in (0.0, 0.25, -0.25, 0.999, -1.0, 1.3, -2.6, 5.5, -14.2):
+        g = rng.standard_normal(n)
+        out = oracle.sweep_pencils(g[None], np.array([alpha]), -1.0, q, periodic)[0]   # alpha = -(a*scale)
+        ref = scipy_pencil(g, alpha, q, periodic)
+        assert np.max(np.abs(out - ref)) < 5e-13 * np.max(np.abs(g)), (q, periodic, alpha)
+
+
+def test_pencil_against_exact_rational_matrix():
+    """n = 8..12, integer data, alpha = 3/8 and -11/8: exact matrix-vector product in rationals."""
+    for n, q in ((8, 8), (10, 6), (12, 10)):
+        rng = np.random.default_rng(n)
+        g = rng.integers(-50, 50, size=n)
+        for alpha in (Fraction(3, 8), Fraction(-11, 8)):
+            k = math.floor(alpha)
+            w = exact_weights(q, alpha - k)
+            for periodic in (True, False):
+                ref = []
+                for j in range(n):
+                    acc = Fraction(0)
+                    for mi, m in enumerate(range(-q // 2 + 1, q // 2 + 1)):
+                        jj = j + k + m
+                        if periodic:
+                            acc += w[mi] * int(g[jj % n])
+                        elif 0 <= jj < n:
+                            acc += w[mi] * int(g[jj])
+                    ref.append(float(acc))
+                out = oracle.sweep_pencils(g[None].astype(float), np.array([float(alpha)]), -1.0, q, periodic)[0]
+                assert np.max(np.abs(out - np.array(ref))) < 1e-13 * 50
+
+
+def test_sweep_indexing_every_dim_and_mask():
+    """6-D sweep == per-pencil routine on explicitly gathered pencils, with the source indexed by a
+    different coordinate subset each time (transposed / mis-strided src or f indexing fails here)."""
+    n = [4, 5, 6, 7, 8, 9]
+    rng = np.random.default_rng(3)
+    f = rng.random(n)
+    for dim in range(6):
+        for mask_dims in ([(dim + 3) % 6], [d for d in range(6) if d != dim], [d for d in (0, 2, 5) if d != dim]):
+            mask = sum(1 << d for d in mask_dims)
+            sshape = [n[d] for d in sorted(mask_dims)]
+            src = rng.uniform(-2.5, 2.5, size=sshape)
+            out = oracle.sweep(f, dim, src, mask, 1.0, 6)
+            # reference: move `dim` last, broadcast src to pencil shape
+            bshape = [n[d] if d in mask_dims else 1 for d in range(6)]
+            a = np.broadcast_to(src.reshape(bshape), n)
+            a_p = np.moveaxis(a, dim, -1)[..., 0].reshape(-1)
+            g_p = np.moveaxis(f, dim, -1).reshape(-1, n[dim])
+            ref = oracle.sweep_pencils(g_p, a_p, 1.0, 6, periodic=dim < 3)
+            ref = np.moveaxis(ref.reshape([n[d] for d in range(6) if d != dim] + [n[dim]]), -1, dim)
+            assert np.array_equal(out, ref), (dim, mask_dims)
+            # and the pencil routine itself is pinned to scipy on a few of those pencils
+            for p in (0, len(a_p) // 2, len(a_p) - 1):
+                assert np.max(np.abs(ref_p(g_p[p], -a_p[p], 6, dim < 3) - oracle.sweep_pencils(
+                    g_p[p:p + 1], a_p[p:p + 1], 1.0, 6, dim < 3)[0])) < 1e-13
+
+
+def ref_p(g, alpha, q, periodic):
+    return scipy_pencil(g, alpha, q, periodic)
+
+
+def test_inplace_equals_out_of_place():
+    rng = np.random.default_rng(5)
+    f = rng.random([6, 6, 6, 6, 6, 6])
+    src = rng.uniform(-1, 1, size=6)
+    for dim in (0, 4):
+        out = oracle.sweep(f, dim, src, 1 << ((dim + 3) % 6), 1.3, 6)
+        g = f.copy()
+        oracle.sweep(g, dim, src, 1 << ((dim + 3) % 6), 1.3, 6, out=g)
+        assert np.array_equal(out, g)
+
+
+# ------------------------------------------------------------------------------------------------
+# property 4: free streaming of a Gaussian matches f0(x - v t, v)  (eq (3): dX/dt = V)
+# ------------------------------------------------------------------------------------------------
+def _free_stream_error(N, q, nsteps=40, dt=0.05):
+    L, vmax, nv = 4 * math.pi, 6.0, 8
+    g = small_grid([N, 1, 1, nv, 1, 1], L, vmax)
+    x, v = g.nodes(0), g.nodes(3)
+    sig, x0 = L / 16.0, L / 3.0
+
+    def f0(xx):                                        # periodised Gaussian
+        return sum(np.exp(-0.5 * ((xx - x0 + kk * L) / sig) ** 2) for kk in range(-6, 7))
+
+    f = (f0(x)[:, None] * np.ones(nv)[None, :]).reshape(g.n).copy()
+    for _ in range(nsteps):
+        f = oracle.advect(g, q - 1, f, 0, None, dt)
+    t = nsteps * dt
+    exact = f0(x[:, None] - v[None, :] * t).reshape(g.n)
+    return np.max(np.abs(f - exact))
+
+
+@pytest.mark.parametrize("q", (6, 8, 10))
+def test_free_streaming_gaussian_convergence(q):
+    e1, e2 = _free_stream_error(64, q), _free_stream_error(128, q)     # sigma/dx = 4 -> 8
+    assert e1 < 2e-3, e1                                              # right sign, right distance
+    assert e2 < 2e-5, e2
+    assert e1 / e2 > 2.0 ** (q - 1.5), (e1, e2, e1 / e2)              # order ~ q
+
+
+def test_free_streaming_wrong_sign_would_fail():
+    """Sanity of the pin itself: streaming with -dt is O(1) away from the closed form."""
+    L, nv, N = 4 * math.pi, 8, 64
+    g = small_grid([N, 1, 1, nv, 1, 1], L, 6.0)
+    x = g.nodes(0)
+    f0 = np.exp(-0.5 * ((x - L / 3) / (L / 16)) ** 2)
+    f = (f0[:, None] * np.ones(nv)).reshape(g.n).copy()
+    a = oracle.advect(g, 7, f, 0, None, 0.4)
+    b = oracle.advect(g, 7, f, 0, None, -0.4)
+    assert np.max(np.abs(a - b)) > 0.3
+
+
+# ------------------------------------------------------------------------------------------------
+# rotation (BASELINE.json configs[3]; eq (3): dV/dt = V x B)
+# ------------------------------------------------------------------------------------------------
+def test_shear_product_is_rotation_matrix():
+    for th in (0.05, 0.1, 2 * math.pi / 63, -0.3, 1.2):
+        t, s = math.tan(th / 2), math.sin(th)
+        Sx = np.array([[1.0, -t], [0.0, 1.0]])          # v1 <- v1 - t v2
+        Sy = np.array([[1.0, 0.0], [s, 1.0]])           # v2 <- v2 + s v1
+        R = np.array([[math.cos(th), -math.sin(th)], [math.sin(th), math.cos(th)]])
+        assert np.max(np.abs(Sx @ Sy @ Sx - R)) < 4e-16
+
+
+def _blob(v1, v2, c=(1.5, 0.5), sig=0.9):
+    return np.exp(-0.5 * (((v1 - c[0]) / sig) ** 2 + ((v2 - c[1]) / sig) ** 2))
+
+
+@pytest.mark.parametrize("axis", (0, 1, 2))
+@pytest.mark.parametrize("theta", (0.1, -0.25))
+def test_rotation_closed_form(axis, theta):
+    """f_new(v) = f_old(R(theta) v) in the plane (a,b) = cyclic successors of the B axis."""
+    nv = 64
+    n = [1, 1, 1, nv, nv, nv]
+    n[3 + axis] = 1
+    g = small_grid(n, vmax=6.0)
+    a, b = (axis + 1) % 3, (axis + 2) % 3
+    va, vb = g.nodes(3 + a), g.nodes(3 + b)
+    shape = [1, 1, 1, 1, 1, 1]
+    sa, sb = list(shape), list(shape)
+    sa[3 + a] = nv; sb[3 + b] = nv
+    VA, VB = va.reshape(sa), vb.reshape(sb)
+    f0 = np.ascontiguousarray(np.broadcast_to(_blob(VA, VB), n))
+    B = [0.0, 0.0, 0.0]; B[axis] = theta / 0.5
+    out = oracle.rotate(g, 7, f0, B, 0.5)
+    c, s = math.cos(theta), math.sin(theta)
+    exact = _blob(c * VA - s * VB, s * VA + c * VB)
+    err = np.max(np.abs(out - exact))
+    wrong = np.max(np.abs(out - _blob(c * VA + s * VB, -s * VA + c * VB)))
+    assert err < 1e-5, err                              # interpolation error of 3 q=8 sweeps at sigma/dv = 4.8
+    assert wrong > 0.05                                 # the other rotation sense is far away
+
+
+def _rotation_return_error(nv, q, nsteps=63):
+    g = small_grid([1, 1, 1, nv, nv, 1], vmax=6.0)
+    v1, v2 = g.nodes(3)[:, None], g.nodes(4)[None, :]
+    f0 = np.exp(-0.5 * v1 ** 2 - v2 ** 2 / 0.5).reshape(g.n).copy()      # C4's anisotropic Gaussian
+    f = f0.copy()
+    th = 2 * math.pi / nsteps                                           # reading S7
+    for _ in range(nsteps):
+        f = oracle.rotate(g, q - 1, f, [0.0, 0.0, 1.0], th)
+    return np.max(np.abs(f - f0)) / np.max(np.abs(f0))
+
+
+def test_rotation_2pi_return():
+    """property 5: n steps totalling 2*pi return f to within interpolation error (and converge with nv)."""
+    e32, e64, e128 = (_rotation_return_error(nv, 8) for nv in (32, 64, 128))
+    assert e32 < 0.06 and e64 < 2e-3 and e128 < 2e-5, (e32, e64, e128)
+    assert e32 / e64 > 10 and e64 / e128 > 30
+    # half the angle does NOT return (the test can fail)
+    g = small_grid([1, 1, 1, 64, 64, 1])
+    v1, v2 = g.nodes(3)[:, None], g.nodes(4)[None, :]
+    f0 = np.exp(-0.5 * v1 ** 2 - v2 ** 2 / 0.5).reshape(g.n).copy()
+    f = f0.copy()
+    for _ in range(16):
+        f = oracle.rotate(g, 7, f, [0.0, 0.0, 1.0], 2 * math.pi / 64)
+    assert np.max(np.abs(f - f0)) > 0.1
+
+
+def test_rotate_rejects_oblique_B_and_identity_for_zero_B():
+    g = small_grid([1, 1, 1, 8, 8, 8])
+    f = np.random.default_rng(0).random(g.n)
+    with pytest.raises(ValueError):
+        oracle.rotate(g, 7, f, [0.1, 0.2, 0.0], 0.1)
+    assert np.array_equal(oracle.rotate(g, 7, f, [0.0, 0.0, 0.0], 0.1), f)
+
+
+# ------------------------------------------------------------------------------------------------
+# density (eq (2))
+# ------------------------------------------------------------------------------------------------
+def test_density_bruteforce_fsum():
+    g = small_grid([3, 2, 4, 5, 6, 7])
+    rng = np.random.default_rng(11)
+    f = rng.random(g.n) * 10.0 ** rng.integers(-8, 8, size=g.n)          # badly scaled on purpose
+    rho = oracle.density(g, f)
+    dv3 = g.dx[3] * g.dx[4] * g.dx[5]
+    for ix in np.ndindex(3, 2, 4):
+        ref = dv3 * math.fsum(f[ix].reshape(-1).tolist())
+        assert abs(rho[ix] - ref) <= 2 * np.spacing(abs(ref))
+
+
+def test_density_maxwellian_closed_form():
+    g = small_grid([16, 2, 2, 32, 32, 32])
+    x1 = g.nodes(0)
+    v = [g.nodes(3 + d) for d in range(3)]
+    M = (2 * math.pi) ** -1.5 * np.exp(-0.5 * (v[0][:, None, None] ** 2 + v[1][None, :, None] ** 2 + v[2][None, None, :] ** 2))
+    fx = 1.0 + 0.01 * np.cos(0.5 * x1)
+    f = np.ascontiguousarray(np.broadcast_to(fx[:, None, None, None, None, None] * M[None, None, None], g.n))
+    rho = oracle.density(g, f)
+    # trapezoid on a Gaussian is spectrally accurate; truncation at |v|=6 is erf(6/sqrt2)^3 - 1 ~ -6e-9
+    assert np.max(np.abs(rho - fx[:, None, None])) < 1e-7
+
+
+# ------------------------------------------------------------------------------------------------
+# named sweeps and the Strang step
+# ------------------------------------------------------------------------------------------------
+def test_advect_E_sweep_closed_form():
+    """Uniform field: f_new(v) = f_old(v - E dt)  (dV/dt = (q/m)E)."""
+    g = small_grid([2, 2, 2, 1, 64, 1])
+    v2 = g.nodes(4)
+    f0 = lambda v: np.exp(-0.5 * ((v - 0.4) / 0.8) ** 2)
+    f = np.ascontiguousarray(np.broadcast_to(f0(v2)[None, None, None, None, :, None], g.n))
+    E = np.full((2, 2, 2), 0.7)
+    E[1, 0, 1] = -1.1
+    out = oracle.advect(g, 7, f, 4, E, 0.3)
+    for ix in np.ndindex(2, 2, 2):
+        # 1e-6: the zero extension at v = +6 truncates a tail of size ~7e-7; a wrong sign is 0.1 away
+        assert np.max(np.abs(out[ix][0, :, 0] - f0(v2 - E[ix] * 0.3))) < 1e-6
+        assert np.max(np.abs(out[ix][0, :, 0] - f0(v2 + E[ix] * 0.3))) > 0.05
+
+
+def test_strang_step_is_the_stated_sequence():
+    g = small_grid([8, 8, 8, 8, 8, 8])
+    rng = np.random.default_rng(2)
+    f = rng.random(g.n)
+    E = [0.3 * rng.standard_normal((8, 8, 8)) for _ in range(3)]
+    B, dt = [0.0, 0.0, 0.8], 0.07
+    ref = f.copy()
+    for d in range(3):
+        ref = oracle.advect(g, 7, ref, d, None, 0.5 * dt)
+    for d in range(3):
+        ref = oracle.advect(g, 7, ref, 3 + d, E[d], dt)
+    ref = oracle.rotate(g, 7, ref, B, dt)
+    for d in range(3):
+        ref = oracle.advect(g, 7, ref, d, None, 0.5 * dt)
+    out = oracle.strang_step(g, 7, f.copy(), E, B, dt)
+    assert np.array_equal(out, ref)
+
+
+def test_strang_step_uniform_field_closed_form():
+    """E uniform, B = 0: exact solution of the split step is
+    f_new(x, v) = f0(x - v dt/2 - (v - E dt) dt/2, v - E dt)."""
+    L = 4 * math.pi
+    g = small_grid([64, 1, 1, 64, 1, 1], L, 6.0)
+    x, v = g.nodes(0)[:, None], g.nodes(3)[None, :]
+    sig = L / 12
+
+    def f0(xx, vv):
+        gx = sum(np.exp(-0.5 * ((xx - L / 2 + kk * L) / sig) ** 2) for kk in range(-4, 5))
+        return gx * np.exp(-0.5 * ((vv - 0.5) / 0.9) ** 2)
+
+    f = f0(x, v).reshape(g.n).copy()
+    E0, dt = 0.6, 0.25
+    E = [np.full((64, 1, 1), E0), None, None]
+    out = oracle.strang_step(g, 7, f, E, None, dt)
+    exact = f0(x - v * dt / 2 - (v - E0 * dt) * dt / 2, v - E0 * dt).reshape(g.n)
+    assert np.max(np.abs(out - exact)) < 5e-6
