@@ -1,0 +1,130 @@
+/* bsl6d.h -- C ABI of libbsl6d.so: the split 1-D advection sweep of the 6-D backward semi-Lagrangian
+ * Vlasov method of arXiv 2303.05994 ("BSL6D"), hand-written for NVIDIA B200 (sm_100a).
+ *
+ * Citations are lines of the paper text plus the section / equation they fall in; "reading Sx"
+ * refers to the table of readings in DESIGN.md.
+ *
+ * Data model
+ *   f        fp64 distribution function on a 6-D tensor grid, dims d = 0..5 = (x1,x2,x3,v1,v2,v3), extents
+ *            n[d], C order: v3 has unit stride, lin = ((((i1*n1+i2)*n2+i3)*n3+j1)*n4+j2)*n5+j3.  This is a
+ *            contiguous torch tensor of shape (n0,..,n5) and the paper's on-disk / CPU layout.
+ *   nodes    node i of dim d sits at lo[d] + i*dx[d].
+ *   bounds   dims 0-2 are periodic with period n[d]*dx[d]; dims 3-5 are extended by zero outside the grid
+ *            (BASELINE.json north_star; the paper is silent on the v boundary, reading S6).
+ *   stencil  centred Lagrange interpolation of odd degree p on q = p+1 (even) nodes around the foot of the
+ *            characteristic, eq (7), for any displacement (integer part + fraction, reading S2).
+ *
+ * Ownership and execution
+ *   Unless a function says HOST, every f / rho / shift-source pointer is a DEVICE pointer owned by the caller,
+ *   8-byte aligned (16-byte for best speed); the library neither allocates nor frees them.  The context owns
+ *   only small device tables.  Work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as
+ *   void*, NULL = legacy default stream) and the call returns without synchronising.  Functions return 0 or
+ *   a negative BSL6D_E* code; a failed call has enqueued nothing.  No exceptions, no printing, no aborts.
+ *   There is no CPU fallback anywhere: without a CUDA device bsl6d_create fails with BSL6D_ECUDA.
+ *   Preconditions not checked: f finite; |displacement| < 2^30 cells.
+ */
+#ifndef BSL6D_H
+#define BSL6D_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BSL6D_VERSION 100
+
+#if defined(__GNUC__)
+#define BSL6D_API __attribute__((visibility("default")))
+#else
+#define BSL6D_API
+#endif
+
+typedef struct bsl6d_ctx bsl6d_ctx;
+
+typedef struct bsl6d_grid {
+    int32_t n[6];   /* extents, each >= 1 */
+    double lo[6];   /* coordinate of node 0 */
+    double dx[6];   /* node spacing, > 0 */
+} bsl6d_grid;
+
+enum {
+    BSL6D_OK = 0,
+    BSL6D_EINVAL = -1,        /* null pointer, bad extent / spacing / degree / dim / mask, non-finite dt */
+    BSL6D_EALIAS = -2,        /* f_in and f_out overlap partially (exact aliasing f_in == f_out is legal) */
+    BSL6D_EUNSUPPORTED = -3,  /* B with more than one non-zero component; extent too large for on-chip staging */
+    BSL6D_ECUDA = -4,         /* CUDA runtime failure; see bsl6d_last_cuda_error */
+    BSL6D_ENOMEM = -5         /* host or device allocation failed */
+};
+
+/* Create a context for `grid` and Lagrange degree `degree` (odd, 1..11; stencil width q = degree+1).
+ * Uses the current CUDA device.  *out receives the context (HOST pointer, opaque). */
+BSL6D_API int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out);
+BSL6D_API void bsl6d_destroy(bsl6d_ctx* ctx);
+
+/* One 1-D advection sweep along `dim` (eq (5), 74-76: one factor of the split step):
+ *     f_out[p, j] = sum_{m=-q/2+1..q/2} l_m(theta_p) * f_in[p, j + k_p + m],
+ *     alpha_p = -(shift_source[p] * (dt/dx[dim])) cells,  k_p = floor(alpha_p),  theta_p = alpha_p - k_p
+ * for every pencil p (all index combinations of the other five dims).  The foot of the characteristic of
+ * output node j is j + alpha_p (reading S1).
+ *   dim 0..2 (x_d advection, dX/dt = V): shift_source = n[dim+3] doubles, the velocity of each
+ *            v_d node; NULL selects the grid's own nodes lo[dim+3] + i*dx[dim+3].
+ *   dim 3..5 (v_d advection by the electric field, dV/dt = (q/m)E): shift_source = n0*n1*n2 doubles, C order,
+ *            (q/m)*E_{dim-3}(x); NULL is BSL6D_EINVAL.
+ * f_in == f_out is legal (in place). */
+BSL6D_API int bsl6d_advect(bsl6d_ctx* ctx, const double* f_in, double* f_out, int dim,
+                 const double* shift_source, double dt, void* stream);
+
+/* The primitive behind every named sweep: src is a dense C-order DEVICE array over the dims whose bit is set
+ * in src_dim_mask (bit d = dim d; the mask must not contain `dim`; mask 0 = one scalar);
+ * alpha_p = -(src[p] * scale) cells (the shift is a function of a subset D of the coordinates). */
+BSL6D_API int bsl6d_advect_generic(bsl6d_ctx* ctx, const double* f_in, double* f_out, int dim,
+                         const double* src, unsigned src_dim_mask, double scale, void* stream);
+
+/* Rotation of velocity space by the background field, dV/dt = V x B (eq (3)), as three velocity
+ * shears (BASELINE.json configs[3], reading S7): with B (HOST, 3 doubles, = (q/m)*B0) along axis c,
+ * (a,b,c) cyclic, theta = B[c]*dt:  shear v_a by foot displacement -v_b*tan(theta/2), shear v_b by
+ * +v_a*sin(theta), shear v_a again.  Result: f_out(v) = f_in(R(theta) v).  Exactly one component of B may be
+ * non-zero (else BSL6D_EUNSUPPORTED); B == 0 copies f_in to f_out.  Three sweeps: f_in -> f_out, then in place. */
+BSL6D_API int bsl6d_rotate(bsl6d_ctx* ctx, const double* f_in, double* f_out, const double B[3], double dt, void* stream);
+
+/* One Strang-split time step (order per BASELINE.json configs[4], reading S8), result in f:
+ *   x1,x2,x3 with dt/2  ->  v1,v2,v3 with E (dt)  ->  rotation (theta = B_c*dt)  ->  x1,x2,x3 with dt/2.
+ * E: HOST array of three DEVICE pointers ((q/m)E_d over x, C order); a NULL entry skips that sweep, E == NULL
+ * skips all three.  B: HOST, may be NULL (no rotation).  f_tmp: optional second DEVICE buffer of the size of f;
+ * if given the sweeps ping-pong between f and f_tmp, if NULL they run in place.  The numbers are identical. */
+BSL6D_API int bsl6d_strang_step(bsl6d_ctx* ctx, double* f, double* f_tmp, const double* const E[3], const double B[3],
+                      double dt, void* stream);
+
+/* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
+ * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
+BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);
+
+/* ---- end-to-end entry point on HOST buffers -------------------------------------------------------------
+ * Runs a sequence of operations on a distribution function that lives in HOST memory (pinned for full speed):
+ * copies f_in_host to the device, runs the ops back to back on an internal stream, copies the result to
+ * f_out_host (may equal f_in_host) and, for density ops, rho to op.rho_host; synchronises before returning.
+ * Device working buffers are allocated on first use and kept by the context. */
+typedef struct bsl6d_host_op {
+    int32_t kind;                /* 0 = advect, 1 = rotate, 2 = density (of the current state) */
+    int32_t dim;                 /* advect: sweep dim */
+    const double* shift_source;  /* advect: HOST pointer or NULL, sizes as in bsl6d_advect */
+    double dt;                   /* advect, rotate */
+    double B[3];                 /* rotate */
+    double* rho_host;            /* density: HOST output, n0*n1*n2 doubles */
+} bsl6d_host_op;
+BSL6D_API int bsl6d_run_host(bsl6d_ctx* ctx, const double* f_in_host, double* f_out_host,
+                   const bsl6d_host_op* ops, int nops);
+
+/* ---- introspection ------------------------------------------------------------------------------------ */
+BSL6D_API const char* bsl6d_strerror(int code);
+BSL6D_API int bsl6d_last_cuda_error(const bsl6d_ctx* ctx);          /* cudaError_t of the last BSL6D_ECUDA, else 0 */
+BSL6D_API long long bsl6d_launch_count(const bsl6d_ctx* ctx);       /* kernels launched by this context so far */
+/* Name of the kernel variant bsl6d_advect* would launch for `dim` ("strided<N,Q>", "unit<N,Q>", "generic"). */
+BSL6D_API int bsl6d_kernel_name(const bsl6d_ctx* ctx, int dim, char* buf, int buflen);
+BSL6D_API int bsl6d_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BSL6D_H */

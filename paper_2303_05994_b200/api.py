@@ -1,0 +1,226 @@
+"""Thin ctypes binding of libbsl6d.so (include/bsl6d.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels behind the C ABI.  torch is used for device memory and streams, nothing else.
+
+There is no CPU fallback: if the shared library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbsl6d.so")
+
+#: every symbol include/bsl6d.h declares (tests check that the library exports exactly these)
+SYMBOLS = (
+    "bsl6d_create", "bsl6d_destroy", "bsl6d_advect", "bsl6d_advect_generic", "bsl6d_rotate",
+    "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
+    "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version",
+)
+
+OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
+
+
+class Grid(C.Structure):
+    """bsl6d_grid: node i of dim d at lo[d] + i*dx[d]."""
+    _fields_ = [("n", C.c_int32 * 6), ("lo", C.c_double * 6), ("dx", C.c_double * 6)]
+
+
+class HostOp(C.Structure):
+    """bsl6d_host_op."""
+    _fields_ = [("kind", C.c_int32), ("dim", C.c_int32), ("shift_source", C.c_void_p), ("dt", C.c_double),
+                ("B", C.c_double * 3), ("rho_host", C.c_void_p)]
+
+
+class Bsl6dError(RuntimeError):
+    def __init__(self, code: int, what: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{what}: error {code} ({detail})")
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libbsl6d.so (built in-tree by paper_2303_05994_b200.build); raises if it is not there."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: run `python -m paper_2303_05994_b200.build` (there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp = C.c_void_p, C.c_void_p
+    lib.bsl6d_create.argtypes = [C.POINTER(Grid), C.c_int, C.POINTER(vp)]
+    lib.bsl6d_destroy.argtypes = [vp]
+    lib.bsl6d_destroy.restype = None
+    lib.bsl6d_advect.argtypes = [vp, dp, dp, C.c_int, dp, C.c_double, vp]
+    lib.bsl6d_advect_generic.argtypes = [vp, dp, dp, C.c_int, dp, C.c_uint, C.c_double, vp]
+    lib.bsl6d_rotate.argtypes = [vp, dp, dp, C.POINTER(C.c_double), C.c_double, vp]
+    lib.bsl6d_strang_step.argtypes = [vp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, vp]
+    lib.bsl6d_density.argtypes = [vp, dp, dp, vp]
+    lib.bsl6d_run_host.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int]
+    lib.bsl6d_strerror.argtypes = [C.c_int]
+    lib.bsl6d_strerror.restype = C.c_char_p
+    lib.bsl6d_last_cuda_error.argtypes = [vp]
+    lib.bsl6d_launch_count.argtypes = [vp]
+    lib.bsl6d_launch_count.restype = C.c_longlong
+    lib.bsl6d_kernel_name.argtypes = [vp, C.c_int, C.c_char_p, C.c_int]
+    lib.bsl6d_version.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _dev_ptr(t: Optional[torch.Tensor], what: str) -> Optional[int]:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{what}: want a contiguous float64 CUDA tensor")
+    return t.data_ptr()
+
+
+def _host_ptr(t: Optional[torch.Tensor], what: str) -> Optional[int]:
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{what}: want a contiguous float64 CPU tensor")
+    return t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+class Context:
+    """bsl6d_ctx*.  Methods carry the names of the C entry points."""
+
+    def __init__(self, n: Sequence[int], lo: Sequence[float], dx: Sequence[float], degree: int):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        g = Grid()
+        for d in range(6):
+            g.n[d], g.lo[d], g.dx[d] = int(n[d]), float(lo[d]), float(dx[d])
+        self.n = tuple(int(v) for v in n)
+        self.degree = int(degree)
+        rc = self._lib.bsl6d_create(C.byref(g), int(degree), C.byref(self._h))
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise Bsl6dError(rc, "bsl6d_create", self._lib.bsl6d_strerror(rc).decode())
+
+    # -- plumbing ---------------------------------------------------------------------------------------
+    def _check(self, rc: int, what: str):
+        if rc != OK:
+            detail = self._lib.bsl6d_strerror(rc).decode()
+            if rc == ECUDA:
+                detail += f"; cudaError {self._lib.bsl6d_last_cuda_error(self._h)}"
+            raise Bsl6dError(rc, what, detail)
+
+    def destroy(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.bsl6d_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def _shape_ok(self, t: torch.Tensor, what: str):
+        if t.numel() != int(torch.tensor(self.n).prod()):
+            raise ValueError(f"{what}: wrong number of elements for grid {self.n}")
+
+    # -- the C entry points -------------------------------------------------------------------------------
+    def advect(self, f_in, f_out, dim: int, shift_source, dt: float, stream=None):
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        self._check(self._lib.bsl6d_advect(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"), int(dim),
+                                           _dev_ptr(shift_source, "shift_source"), float(dt), _stream(stream)),
+                    "bsl6d_advect")
+        return f_out
+
+    def advect_generic(self, f_in, f_out, dim: int, src, src_dim_mask: int, scale: float, stream=None):
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        want = 1
+        for d in range(6):
+            if src_dim_mask >> d & 1:
+                want *= self.n[d]
+        if src is not None and src.numel() != want:
+            raise ValueError("src: wrong number of elements for the mask")
+        self._check(self._lib.bsl6d_advect_generic(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"),
+                                                   int(dim), _dev_ptr(src, "src"), int(src_dim_mask), float(scale),
+                                                   _stream(stream)), "bsl6d_advect_generic")
+        return f_out
+
+    def rotate(self, f_in, f_out, B: Sequence[float], dt: float, stream=None):
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        Bc = (C.c_double * 3)(*[float(b) for b in B])
+        self._check(self._lib.bsl6d_rotate(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"), Bc, float(dt),
+                                           _stream(stream)), "bsl6d_rotate")
+        return f_out
+
+    def strang_step(self, f, f_tmp, E, B, dt: float, stream=None):
+        self._shape_ok(f, "f")
+        Ep = None
+        if E is not None:
+            Ep = (C.c_void_p * 3)(*[_dev_ptr(e, "E") for e in E])
+        Bc = None if B is None else (C.c_double * 3)(*[float(b) for b in B])
+        self._check(self._lib.bsl6d_strang_step(self._h, _dev_ptr(f, "f"), _dev_ptr(f_tmp, "f_tmp"), Ep, Bc, float(dt),
+                                                _stream(stream)), "bsl6d_strang_step")
+        return f
+
+    def density(self, f, rho, stream=None):
+        self._shape_ok(f, "f")
+        if rho.numel() != self.n[0] * self.n[1] * self.n[2]:
+            raise ValueError("rho: wrong number of elements")
+        self._check(self._lib.bsl6d_density(self._h, _dev_ptr(f, "f"), _dev_ptr(rho, "rho"), _stream(stream)),
+                    "bsl6d_density")
+        return rho
+
+    def run_host(self, f_in_host, f_out_host, ops: Sequence[dict]):
+        """ops: dicts with kind in {'advect','rotate','density'} and dim / shift_source / dt / B / rho_host."""
+        self._shape_ok(f_in_host, "f_in_host"); self._shape_ok(f_out_host, "f_out_host")
+        arr = (HostOp * max(1, len(ops)))()
+        keep = []
+        for i, op in enumerate(ops):
+            kind = {"advect": 0, "rotate": 1, "density": 2}[op["kind"]]
+            arr[i].kind = kind
+            arr[i].dim = int(op.get("dim", 0))
+            arr[i].dt = float(op.get("dt", 0.0))
+            ss = op.get("shift_source")
+            arr[i].shift_source = _host_ptr(ss, "shift_source")
+            rho = op.get("rho_host")
+            arr[i].rho_host = _host_ptr(rho, "rho_host")
+            for k, b in enumerate(op.get("B", (0.0, 0.0, 0.0))):
+                arr[i].B[k] = float(b)
+            keep += [ss, rho]
+        self._check(self._lib.bsl6d_run_host(self._h, _host_ptr(f_in_host, "f_in_host"),
+                                             _host_ptr(f_out_host, "f_out_host"), arr, len(ops)), "bsl6d_run_host")
+        return f_out_host
+
+    # -- introspection --------------------------------------------------------------------------------------
+    def launch_count(self) -> int:
+        return int(self._lib.bsl6d_launch_count(self._h))
+
+    def kernel_name(self, dim: int) -> str:
+        buf = C.create_string_buffer(128)
+        self._check(self._lib.bsl6d_kernel_name(self._h, int(dim), buf, 128), "bsl6d_kernel_name")
+        return buf.value.decode()
+
+
+def create(n, lo, dx, degree) -> Context:
+    return Context(n, lo, dx, degree)
+
+
+def version() -> int:
+    return int(load_library().bsl6d_version())

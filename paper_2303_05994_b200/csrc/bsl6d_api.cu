@@ -1,0 +1,557 @@
+// bsl6d_api.cu -- the C ABI of include/bsl6d.h: argument checks, launch planning, the Strang driver.
+// All arithmetic on f happens in the kernels of sweep_kernels.cuh / density_kernels.cuh.
+#include "../../include/bsl6d.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "density_kernels.cuh"
+#include "sweep_kernels.cuh"
+
+using bsl6d::SweepArgs;
+
+struct bsl6d_ctx {
+    bsl6d_grid g;
+    int q;
+    int device;
+    size_t npts;
+    double* d_nodes;          // 6 node tables back to back (device)
+    size_t node_off[6];
+    double* d_part;           // density partial sums (device), nx * G
+    uint32_t dens_G;
+    size_t dens_chunk;
+    int last_cuda;
+    long long launches;
+    // host-path working set (bsl6d_run_host), allocated on first use
+    double* h_f;              // device buffer for f
+    double* h_small;          // device buffer for shift sources / rho
+    size_t h_small_cap;
+    cudaStream_t h_stream;
+};
+
+namespace {
+
+typedef void (*sweep_fn)(const SweepArgs);
+
+struct KernelChoice {
+    sweep_fn fn;
+    int threads;
+    size_t smem;
+    int kind;                 // 0 strided, 1 unit, 2 generic
+    int gen_T;
+};
+
+template <int N, int Q, bool P>
+constexpr int strided_threads() { return N <= 32 ? 256 : 128; }
+
+template <int N, int Q, bool P>
+KernelChoice strided_choice() {
+    constexpr int T = strided_threads<N, Q, P>();
+    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T>, T, 0, 0, 0};
+}
+
+template <int N, int Q>
+KernelChoice unit_choice() {
+    constexpr int T = 128;
+    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, T>, T, sizeof(double) * T * (N + 1), 1, 0};
+}
+
+template <int N, bool P>
+bool strided_by_q(int q, KernelChoice& c) {
+    switch (q) {
+        case 4: c = strided_choice<N, 4, P>(); return true;
+        case 6: c = strided_choice<N, 6, P>(); return true;
+        case 8: c = strided_choice<N, 8, P>(); return true;
+        case 10: c = strided_choice<N, 10, P>(); return true;
+        default: return false;
+    }
+}
+
+template <bool P>
+bool strided_lookup(int n, int q, KernelChoice& c) {
+    switch (n) {
+        case 8: return strided_by_q<8, P>(q, c);
+        case 16: return strided_by_q<16, P>(q, c);
+        case 32: return strided_by_q<32, P>(q, c);
+        case 48: return strided_by_q<48, P>(q, c);
+        case 64: return strided_by_q<64, P>(q, c);
+        default: return false;
+    }
+}
+
+template <int N>
+bool unit_by_q(int q, KernelChoice& c) {
+    switch (q) {
+        case 4: c = unit_choice<N, 4>(); return true;
+        case 6: c = unit_choice<N, 6>(); return true;
+        case 8: c = unit_choice<N, 8>(); return true;
+        case 10: c = unit_choice<N, 10>(); return true;
+        default: return false;
+    }
+}
+
+bool unit_lookup(int n, int q, KernelChoice& c) {
+    switch (n) {
+        case 8: return unit_by_q<8>(q, c);
+        case 16: return unit_by_q<16>(q, c);
+        case 32: return unit_by_q<32>(q, c);
+        case 48: return unit_by_q<48>(q, c);
+        case 64: return unit_by_q<64>(q, c);
+        default: return false;
+    }
+}
+
+// Which kernel serves a sweep along `dim`?  (Also used by bsl6d_kernel_name.)
+int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
+    const int n = c->g.n[dim];
+    const bool periodic = dim < 3;
+    size_t inner = 1;
+    for (int d = dim + 1; d < 6; ++d) inner *= (size_t)c->g.n[d];
+    bool ok;
+    if (inner == 1) ok = !periodic && unit_lookup(n, c->q, k);
+    else ok = periodic ? strided_lookup<true>(n, c->q, k) : strided_lookup<false>(n, c->q, k);
+    if (ok) return BSL6D_OK;
+    // fallback: column staged in shared memory, n * T doubles
+    const size_t cap = 200 * 1024;
+    int T = 64;
+    if ((size_t)n * T * sizeof(double) > cap) T = 32;
+    if ((size_t)n * T * sizeof(double) > cap) return BSL6D_EUNSUPPORTED;
+    k = KernelChoice{nullptr, T, (size_t)n * T * sizeof(double), 2, T};
+    return BSL6D_OK;
+}
+
+int cuda_fail(bsl6d_ctx* c, cudaError_t e) {
+    if (c) c->last_cuda = (int)e;
+    (void)cudaGetLastError();
+    return BSL6D_ECUDA;
+}
+
+uint32_t ceil_pow2_log2(uint64_t v) {
+    uint32_t l = 0;
+    while ((1ull << l) < v) ++l;
+    return l;
+}
+
+// Build the launch arguments and enqueue one sweep.
+int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const double* src, unsigned mask,
+                 double scale, cudaStream_t stream) {
+    if (!c || !f_in || !f_out || !src) return BSL6D_EINVAL;
+    if (dim < 0 || dim > 5 || (mask & ~0x3Fu) || (mask & (1u << dim))) return BSL6D_EINVAL;
+    if (!std::isfinite(scale)) return BSL6D_EINVAL;
+    const size_t bytes = c->npts * sizeof(double);
+    if (f_in != f_out) {
+        const char* a = (const char*)f_in;
+        const char* b = (const char*)f_out;
+        if (a < b + bytes && b < a + bytes) return BSL6D_EALIAS;
+    }
+    const int32_t* n = c->g.n;
+    size_t inner = 1, outer = 1;
+    for (int d = dim + 1; d < 6; ++d) inner *= (size_t)n[d];
+    for (int d = 0; d < dim; ++d) outer *= (size_t)n[d];
+    if (inner > 0xFFFFFFFFull || outer > 0xFFFFFFFFull || inner * outer > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
+
+    KernelChoice kc;
+    int rc = choose_kernel(c, dim, kc);
+    if (rc) return rc;
+
+    SweepArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.in = f_in;
+    a.out = f_out;
+    a.src = src;
+    a.scale = scale;
+    a.inner = (uint32_t)inner;
+    a.outer = (uint32_t)outer;
+    a.n = (uint32_t)n[dim];
+
+    // ---- source-index terms: runs of adjacent masked dims inside the outer / inner group ----------------
+    size_t sstride[6];
+    {
+        size_t s = 1;
+        for (int d = 5; d >= 0; --d) {
+            if (mask & (1u << d)) { sstride[d] = s; s *= (size_t)n[d]; } else sstride[d] = 0;
+        }
+        if (s > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
+    }
+    for (int grp = 0; grp < 2; ++grp) {
+        const int dlo = grp == 0 ? 0 : dim + 1, dhi = grp == 0 ? dim : 6;   // [dlo, dhi)
+        int d = dhi - 1;
+        size_t below = 1;
+        while (d >= dlo) {
+            if (!(mask & (1u << d))) { below *= (size_t)n[d]; --d; continue; }
+            // run of masked dims d, d-1, ... (towards slower dims)
+            size_t extent = 1;
+            const size_t run_below = below, run_sstride = sstride[d];
+            while (d >= dlo && (mask & (1u << d))) { extent *= (size_t)n[d]; below *= (size_t)n[d]; --d; }
+            const bool slowest = (d < dlo);
+            if (a.nterms >= (uint32_t)bsl6d::kMaxSrcTerms) return BSL6D_EUNSUPPORTED;
+            const uint32_t t = a.nterms++;
+            a.t_inner[t] = (uint32_t)grp;
+            a.t_below[t] = (uint32_t)run_below;
+            a.t_extent[t] = slowest ? 0u : (uint32_t)extent;
+            a.t_sstride[t] = (uint32_t)run_sstride;
+        }
+    }
+
+    // ---- grid -------------------------------------------------------------------------------------------
+    unsigned grid;
+    if (kc.kind == 1) {
+        grid = (unsigned)((outer + kc.threads - 1) / kc.threads);
+    } else {
+        const uint64_t lim = inner < (uint64_t)kc.threads ? inner : (uint64_t)kc.threads;
+        a.ti_log2 = ceil_pow2_log2(lim);
+        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)kc.threads / TI;
+        a.nib = (uint32_t)((inner + TI - 1) / TI);
+        const uint64_t nbo = (outer + TO - 1) / TO;
+        if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+        grid = (unsigned)((uint64_t)a.nib * nbo);
+    }
+
+    cudaError_t e;
+    if (kc.kind == 2) {
+        if (kc.gen_T == 64) {
+            e = cudaFuncSetAttribute(bsl6d::sweep_generic_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)kc.smem);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+            bsl6d::sweep_generic_kernel<64><<<grid, 64, kc.smem, stream>>>(a, c->q, dim < 3 ? 1 : 0);
+        } else {
+            e = cudaFuncSetAttribute(bsl6d::sweep_generic_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)kc.smem);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+            bsl6d::sweep_generic_kernel<32><<<grid, 32, kc.smem, stream>>>(a, c->q, dim < 3 ? 1 : 0);
+        }
+    } else {
+        if (kc.smem > 48 * 1024) {
+            e = cudaFuncSetAttribute((const void*)kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kc.smem);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+        }
+        void* args[] = {(void*)&a};
+        e = cudaLaunchKernel((const void*)kc.fn, dim3(grid), dim3(kc.threads), args, kc.smem, stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
+}
+
+struct Shear { int dim; int src_dim; double scale; };
+
+// Three shears of the rotation (see bsl6d_rotate in the header).  Returns the number of sweeps (0 or 3).
+int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear out[3], int* count) {
+    *count = 0;
+    if (!std::isfinite(dt)) return BSL6D_EINVAL;
+    int ax = -1;
+    for (int i = 0; i < 3; ++i) {
+        if (!std::isfinite(B[i])) return BSL6D_EINVAL;
+        if (B[i] != 0.0) { if (ax >= 0) return BSL6D_EUNSUPPORTED; ax = i; }
+    }
+    if (ax < 0) return BSL6D_OK;
+    const int a = (ax + 1) % 3, b = (ax + 2) % 3;
+    const double theta = B[ax] * dt;
+    const double t = std::tan(0.5 * theta), s = std::sin(theta);
+    out[0] = Shear{3 + a, 3 + b, t / c->g.dx[3 + a]};       // foot displacement -v_b tan(theta/2)
+    out[1] = Shear{3 + b, 3 + a, -s / c->g.dx[3 + b]};      // foot displacement +v_a sin(theta)
+    out[2] = out[0];
+    *count = 3;
+    return BSL6D_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bsl6d_version(void) { return BSL6D_VERSION; }
+
+const char* bsl6d_strerror(int code) {
+    switch (code) {
+        case BSL6D_OK: return "ok";
+        case BSL6D_EINVAL: return "invalid argument";
+        case BSL6D_EALIAS: return "f_in and f_out overlap partially";
+        case BSL6D_EUNSUPPORTED: return "unsupported configuration";
+        case BSL6D_ECUDA: return "CUDA runtime error";
+        case BSL6D_ENOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+
+int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
+    if (!grid || !out) return BSL6D_EINVAL;
+    *out = nullptr;
+    if (degree < 1 || degree > 11 || !(degree & 1)) return BSL6D_EINVAL;
+    size_t npts = 1, nn = 0;
+    for (int d = 0; d < 6; ++d) {
+        if (grid->n[d] < 1 || !(grid->dx[d] > 0.0) || !std::isfinite(grid->dx[d]) || !std::isfinite(grid->lo[d]))
+            return BSL6D_EINVAL;
+        if (npts > (size_t)1 << 40) return BSL6D_EUNSUPPORTED;
+        npts *= (size_t)grid->n[d];
+        nn += (size_t)grid->n[d];
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ECUDA; }
+    bsl6d_ctx* c = new (std::nothrow) bsl6d_ctx();
+    if (!c) return BSL6D_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->g = *grid;
+    c->q = degree + 1;
+    c->device = dev;
+    c->npts = npts;
+
+    std::vector<double> nodes(nn);
+    size_t off = 0;
+    for (int d = 0; d < 6; ++d) {
+        c->node_off[d] = off;
+        for (int i = 0; i < grid->n[d]; ++i) {
+            const double step = (double)i * grid->dx[d];      // one multiply, one add (no contraction: see build flags)
+            nodes[off + i] = grid->lo[d] + step;
+        }
+        off += (size_t)grid->n[d];
+    }
+    e = cudaMalloc((void**)&c->d_nodes, nn * sizeof(double));
+    if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? BSL6D_ENOMEM : BSL6D_ECUDA; }
+    e = cudaMemcpy(c->d_nodes, nodes.data(), nn * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(c->d_nodes); delete c; (void)cudaGetLastError(); return BSL6D_ECUDA; }
+
+    // density plan: chunks of <= 32768 doubles (256 KB) per block
+    const size_t seg = (size_t)grid->n[3] * grid->n[4] * grid->n[5];
+    const size_t nx = (size_t)grid->n[0] * grid->n[1] * grid->n[2];
+    const size_t target = 32768;
+    size_t G = (seg + target - 1) / target;
+    size_t chunk = (seg + G - 1) / G;
+    chunk = (chunk + 1) & ~(size_t)1;                           // even => 16-byte aligned chunks
+    G = (seg + chunk - 1) / chunk;
+    c->dens_G = (uint32_t)G;
+    c->dens_chunk = chunk;
+    if (G > 1) {
+        e = cudaMalloc((void**)&c->d_part, nx * G * sizeof(double));
+        if (e != cudaSuccess) { cudaFree(c->d_nodes); delete c; (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+    }
+    *out = c;
+    return BSL6D_OK;
+}
+
+void bsl6d_destroy(bsl6d_ctx* c) {
+    if (!c) return;
+    if (c->h_stream) { cudaStreamSynchronize(c->h_stream); cudaStreamDestroy(c->h_stream); }
+    cudaFree(c->h_f);
+    cudaFree(c->h_small);
+    cudaFree(c->d_part);
+    cudaFree(c->d_nodes);
+    (void)cudaGetLastError();
+    delete c;
+}
+
+int bsl6d_last_cuda_error(const bsl6d_ctx* c) { return c ? c->last_cuda : 0; }
+long long bsl6d_launch_count(const bsl6d_ctx* c) { return c ? c->launches : 0; }
+
+int bsl6d_kernel_name(const bsl6d_ctx* c, int dim, char* buf, int buflen) {
+    if (!c || !buf || buflen < 1 || dim < 0 || dim > 5) return BSL6D_EINVAL;
+    KernelChoice k;
+    int rc = choose_kernel(c, dim, k);
+    if (rc) return rc;
+    const char* kind = k.kind == 0 ? "strided" : (k.kind == 1 ? "unit" : "generic");
+    std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
+                  dim < 3 ? "periodic" : "zero", k.threads);
+    return BSL6D_OK;
+}
+
+int bsl6d_advect_generic(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const double* src,
+                         unsigned src_dim_mask, double scale, void* stream) {
+    return launch_sweep(c, f_in, f_out, dim, src, src_dim_mask, scale, (cudaStream_t)stream);
+}
+
+int bsl6d_advect(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const double* shift_source, double dt,
+                 void* stream) {
+    if (!c || dim < 0 || dim > 5 || !std::isfinite(dt)) return BSL6D_EINVAL;
+    const double scale = dt / c->g.dx[dim];
+    if (dim < 3) {
+        const double* s = shift_source ? shift_source : c->d_nodes + c->node_off[dim + 3];
+        return launch_sweep(c, f_in, f_out, dim, s, 1u << (dim + 3), scale, (cudaStream_t)stream);
+    }
+    if (!shift_source) return BSL6D_EINVAL;
+    return launch_sweep(c, f_in, f_out, dim, shift_source, 0x7u, scale, (cudaStream_t)stream);
+}
+
+int bsl6d_rotate(bsl6d_ctx* c, const double* f_in, double* f_out, const double B[3], double dt, void* stream) {
+    if (!c || !f_in || !f_out || !B) return BSL6D_EINVAL;
+    Shear sh[3];
+    int cnt = 0;
+    int rc = plan_rotation(c, B, dt, sh, &cnt);
+    if (rc) return rc;
+    const size_t bytes = c->npts * sizeof(double);
+    if (f_in != f_out) {
+        const char* a = (const char*)f_in;
+        const char* b = (const char*)f_out;
+        if (a < b + bytes && b < a + bytes) return BSL6D_EALIAS;
+    }
+    if (cnt == 0) {
+        if (f_in != f_out) {
+            cudaError_t e = cudaMemcpyAsync(f_out, f_in, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+        }
+        return BSL6D_OK;
+    }
+    const double* cur = f_in;
+    for (int i = 0; i < 3; ++i) {
+        rc = launch_sweep(c, cur, f_out, sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim,
+                          sh[i].scale, (cudaStream_t)stream);
+        if (rc) return rc;
+        cur = f_out;
+    }
+    return BSL6D_OK;
+}
+
+int bsl6d_strang_step(bsl6d_ctx* c, double* f, double* f_tmp, const double* const E[3], const double B[3], double dt,
+                      void* stream) {
+    if (!c || !f || !std::isfinite(dt)) return BSL6D_EINVAL;
+    struct Step { int dim; const double* src; unsigned mask; double scale; };
+    Step steps[12];
+    int ns = 0;
+    const double half = 0.5 * dt;
+    for (int d = 0; d < 3; ++d)
+        steps[ns++] = Step{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+    if (E)
+        for (int d = 0; d < 3; ++d)
+            if (E[d]) steps[ns++] = Step{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
+    if (B) {
+        Shear sh[3];
+        int cnt = 0;
+        int rc = plan_rotation(c, B, dt, sh, &cnt);
+        if (rc) return rc;
+        for (int i = 0; i < cnt; ++i)
+            steps[ns++] = Step{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
+    }
+    for (int d = 0; d < 3; ++d)
+        steps[ns++] = Step{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+
+    if (f_tmp) {
+        const size_t bytes = c->npts * sizeof(double);
+        const char* a = (const char*)f;
+        const char* b = (const char*)f_tmp;
+        if (a < b + bytes && b < a + bytes) return BSL6D_EALIAS;
+    }
+    // ping-pong f -> f_tmp -> f ...; with an odd number of sweeps the first one runs in place so that the
+    // result lands in f.  Without f_tmp everything runs in place.
+    double* cur = f;
+    double* other = f_tmp;
+    for (int s = 0; s < ns; ++s) {
+        double* dst = cur;
+        if (other && !((ns & 1) && s == 0)) dst = other;
+        int rc = launch_sweep(c, cur, dst, steps[s].dim, steps[s].src, steps[s].mask, steps[s].scale,
+                              (cudaStream_t)stream);
+        if (rc) return rc;
+        if (dst != cur) { other = cur; cur = dst; }
+    }
+    return BSL6D_OK;
+}
+
+int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
+    if (!c || !f || !rho) return BSL6D_EINVAL;
+    const bsl6d_grid& g = c->g;
+    const size_t seg = (size_t)g.n[3] * g.n[4] * g.n[5];
+    const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
+    const double dv3 = g.dx[3] * g.dx[4] * g.dx[5];
+    const uint32_t G = c->dens_G;
+    if (nx * G > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+    const bool vec = (seg % 2 == 0) && (((uintptr_t)f & 15u) == 0);
+    double* out = G == 1 ? rho : c->d_part;
+    constexpr int T = 256;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (vec) bsl6d::density_kernel<T, true><<<(unsigned)(nx * G), T, 0, st>>>(f, out, seg, G, c->dens_chunk, dv3);
+    else bsl6d::density_kernel<T, false><<<(unsigned)(nx * G), T, 0, st>>>(f, out, seg, G, c->dens_chunk, dv3);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    if (G > 1) {
+        bsl6d::density_finish_kernel<<<(unsigned)((nx + 255) / 256), 256, 0, st>>>(c->d_part, rho, nx, G, dv3);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(c, e);
+        c->launches += 1;
+    }
+    return BSL6D_OK;
+}
+
+int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, const bsl6d_host_op* ops, int nops) {
+    if (!c || !f_in_host || !f_out_host || nops < 0 || (nops > 0 && !ops)) return BSL6D_EINVAL;
+    const bsl6d_grid& g = c->g;
+    const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
+    const size_t bytes = c->npts * sizeof(double);
+    // validate + size the small-buffer arena (one slot per op so that nothing in flight is overwritten)
+    size_t small = 0;
+    for (int i = 0; i < nops; ++i) {
+        const bsl6d_host_op& op = ops[i];
+        if (op.kind == 0) {
+            if (op.dim < 0 || op.dim > 5 || !std::isfinite(op.dt)) return BSL6D_EINVAL;
+            if (op.dim >= 3 && !op.shift_source) return BSL6D_EINVAL;
+            if (op.shift_source) small += op.dim < 3 ? (size_t)g.n[op.dim + 3] : nx;
+        } else if (op.kind == 1) {
+            Shear sh[3];
+            int cnt;
+            int rc = plan_rotation(c, op.B, op.dt, sh, &cnt);
+            if (rc) return rc;
+        } else if (op.kind == 2) {
+            if (!op.rho_host) return BSL6D_EINVAL;
+            small += nx;
+        } else {
+            return BSL6D_EINVAL;
+        }
+    }
+    cudaError_t e;
+    if (!c->h_stream) {
+        e = cudaStreamCreateWithFlags(&c->h_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+    if (!c->h_f) {
+        e = cudaMalloc((void**)&c->h_f, bytes);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); c->h_f = nullptr; return BSL6D_ENOMEM; }
+    }
+    if (small > c->h_small_cap) {
+        cudaFree(c->h_small);
+        c->h_small = nullptr;
+        c->h_small_cap = 0;
+        e = cudaMalloc((void**)&c->h_small, small * sizeof(double));
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+        c->h_small_cap = small;
+    }
+    cudaStream_t st = c->h_stream;
+    e = cudaMemcpyAsync(c->h_f, f_in_host, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    size_t off = 0;
+    int rc = BSL6D_OK;
+    for (int i = 0; i < nops && rc == BSL6D_OK; ++i) {
+        const bsl6d_host_op& op = ops[i];
+        if (op.kind == 0) {
+            const double* dsrc = nullptr;
+            if (op.shift_source) {
+                const size_t cnt = op.dim < 3 ? (size_t)g.n[op.dim + 3] : nx;
+                e = cudaMemcpyAsync(c->h_small + off, op.shift_source, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
+                if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
+                dsrc = c->h_small + off;
+                off += cnt;
+            }
+            rc = bsl6d_advect(c, c->h_f, c->h_f, op.dim, dsrc, op.dt, st);
+        } else if (op.kind == 1) {
+            rc = bsl6d_rotate(c, c->h_f, c->h_f, op.B, op.dt, st);
+        } else {
+            rc = bsl6d_density(c, c->h_f, c->h_small + off, st);
+            if (rc == BSL6D_OK) {
+                e = cudaMemcpyAsync(op.rho_host, c->h_small + off, nx * sizeof(double), cudaMemcpyDeviceToHost, st);
+                if (e != cudaSuccess) rc = cuda_fail(c, e);
+            }
+            off += nx;
+        }
+    }
+    if (rc == BSL6D_OK) {
+        e = cudaMemcpyAsync(f_out_host, c->h_f, bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) rc = cuda_fail(c, e);
+    }
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess && rc == BSL6D_OK) rc = cuda_fail(c, e);
+    return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,265 @@
+// sweep_kernels.cuh -- device code of the 1-D advection sweep (sm_100a).
+//
+// One sweep = for every pencil p along the swept dim:  out[p,j] = sum_m l_m(theta_p) * in[p, j+k_p+m]
+// (eq (7), 69-72 eq (5); include/bsl6d.h).  The 6-D array is viewed as [outer][N][inner].
+//
+// Design: a pencil is owned by exactly ONE thread, which
+//   1. evaluates the shift of its pencil (a1) and the q Lagrange weights (a2) in registers,
+//   2. loads the whole pencil into registers *in shifted order*: register t holds in[(r0+t) mod N]
+//      (periodic) or in[r0+t]-or-zero (zero extension) with r0 = k - q/2 + 1, so the data-dependent
+//      displacement k only ever appears in a load ADDRESS,
+//   3. forms out[j] = sum_{m'} w[m'] * u[j+m'] with compile-time register indices (fully unrolled) and
+//      streams the results out.
+// Every element of f is therefore read once and written once (16 B/point), no halo is re-read, and because
+// all loads of a pencil precede its stores, f_in == f_out is safe.
+//   * strided dims (inner > 1): lanes run along `inner`, so every load/store instruction of a warp is one
+//     contiguous 256 B segment per pencil row -- no shared memory at all.
+//   * unit-stride dim (inner == 1): a block first transposes T pencils through padded shared memory.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace bsl6d {
+
+constexpr int kMaxSrcTerms = 5;
+
+struct SweepArgs {
+    const double* in;
+    double* out;
+    const double* src;     // shift source (device), indexed by the terms below
+    double scale;          // alpha_cells = -(src * scale)
+    uint32_t inner;        // product of extents of dims faster than the swept one
+    uint32_t outer;        // product of extents of dims slower than the swept one
+    uint32_t n;            // extent of the swept dim (== template N in the specialised kernels)
+    uint32_t ti_log2;      // strided: threads of a block along `inner` = 1 << ti_log2
+    uint32_t nib;          // strided: number of inner chunks (= ceil(inner / TI))
+    uint32_t nterms;       // src index = sum_t ((g_t / below_t) % extent_t) * sstride_t,  g_t = outer or inner index
+    uint32_t t_inner[kMaxSrcTerms];   // 1: term decodes the inner index, 0: the outer index
+    uint32_t t_below[kMaxSrcTerms];
+    uint32_t t_extent[kMaxSrcTerms];
+    uint32_t t_sstride[kMaxSrcTerms];
+};
+
+// ---- a2: Lagrange basis on the nodes m_i = i - Q/2 + 1, i = 0..Q-1 ------------------------------------------
+// w_i = prod_{j != i} (theta - m_j) / prod_{j != i} (m_i - m_j).  Numerators by prefix/suffix products
+// (3Q multiplies), denominators (-1)^(Q-1-i) i! (Q-1-i)! folded into compile-time reciprocals.  theta == 0 and
+// theta == 1 are mapped to exact unit vectors so that integer-cell shifts are exact permutations (reading S11).
+template <int Q>
+struct LagrangeDen {
+    double r[Q];
+    constexpr LagrangeDen() : r() {
+        for (int i = 0; i < Q; ++i) {
+            double d = 1.0;
+            for (int j = 0; j < Q; ++j)
+                if (j != i) d *= (double)(i - j);
+            r[i] = 1.0 / d;
+        }
+    }
+};
+
+template <int Q>
+__device__ __forceinline__ void lagrange_weights(double theta, double (&w)[Q]) {
+    constexpr LagrangeDen<Q> den{};
+    double d[Q], pre[Q], suf[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) d[i] = theta - (double)(i - Q / 2 + 1);
+    pre[0] = 1.0;
+#pragma unroll
+    for (int i = 1; i < Q; ++i) pre[i] = pre[i - 1] * d[i - 1];
+    suf[Q - 1] = 1.0;
+#pragma unroll
+    for (int i = Q - 2; i >= 0; --i) suf[i] = suf[i + 1] * d[i + 1];
+    const bool at0 = (theta == 0.0), at1 = (theta == 1.0);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+        double v = (pre[i] * suf[i]) * den.r[i];
+        if (at0) v = (i == Q / 2 - 1) ? 1.0 : 0.0;
+        if (at1) v = (i == Q / 2) ? 1.0 : 0.0;
+        w[i] = v;
+    }
+}
+
+// ---- a1: displacement of one pencil -> integer part k and fraction theta -----------------------------------
+__device__ __forceinline__ void split_shift(double a, double scale, long long& k, double& theta) {
+    const double alpha = -(a * scale);
+    double kf = floor(alpha);
+    theta = alpha - kf;                                   // exact; in [0,1]
+    kf = fmin(fmax(kf, -4.0e18), 4.0e18);
+    k = (long long)kf;
+}
+
+__device__ __forceinline__ uint32_t src_offset(const SweepArgs& a, uint32_t o, uint32_t i) {
+    uint32_t off = 0;
+    for (uint32_t t = 0; t < a.nterms; ++t) {
+        uint32_t g = a.t_inner[t] ? i : o;
+        if (a.t_below[t] != 1u) g /= a.t_below[t];
+        if (a.t_extent[t] != 0u) g %= a.t_extent[t];      // extent 0 = "slowest term of its group": no wrap needed
+        off += g * a.t_sstride[t];
+    }
+    return off;
+}
+
+// ---- a4: strided sweep, one column per thread, no shared memory --------------------------------------------
+template <int N, int Q, bool PERIODIC, int T>
+__global__ void __launch_bounds__(T) sweep_strided_kernel(const SweepArgs a) {
+    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
+    const uint32_t bo = blockIdx.x / a.nib;
+    const uint32_t bi = blockIdx.x - bo * a.nib;
+    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
+    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
+    if (i >= a.inner || o >= a.outer) return;
+
+    long long k;
+    double theta;
+    split_shift(__ldg(a.src + src_offset(a, o, i)), a.scale, k, theta);
+
+    const size_t stride = a.inner;
+    const size_t base = (size_t)o * N * stride + i;
+    const double* __restrict__ pin = a.in + base;
+    double* pout = a.out + base;
+
+    constexpr int NU = PERIODIC ? N : N + Q - 1;
+    double u[NU];
+    if (PERIODIC) {
+        int r0 = (int)((k + (long long)(1 - Q / 2)) % (long long)N);
+        if (r0 < 0) r0 += N;
+#pragma unroll
+        for (int t = 0; t < N; ++t) {
+            int row = r0 + t;
+            if (row >= N) row -= N;
+            u[t] = __ldcs(pin + (size_t)row * stride);
+        }
+    } else {
+        // rows r0 .. r0+N+Q-2; anything outside [0,N) is the zero extension
+        long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
+        kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
+        const int r0 = (int)kc + (1 - Q / 2);
+#pragma unroll
+        for (int t = 0; t < NU; ++t) {
+            const int row = r0 + t;
+            u[t] = (row >= 0 && row < N) ? __ldcs(pin + (size_t)row * stride) : 0.0;
+        }
+    }
+
+    double w[Q];
+    lagrange_weights<Q>(theta, w);
+
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double acc = w[0] * u[PERIODIC ? (j % N) : j];
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[PERIODIC ? ((j + m) % N) : (j + m)], acc);
+        __stcs(pout + (size_t)j * stride, acc);
+    }
+}
+
+// ---- a3: unit-stride sweep (swept dim is the contiguous one; always a v dim => zero extension) -------------
+// A block owns T consecutive pencils = one contiguous chunk of T*N doubles.  Coalesced load -> padded smem
+// (row stride N+1 doubles: conflict-free for "lane = pencil" access) -> each thread reads ITS pencil in shifted
+// order into registers -> results back into the same smem row -> coalesced store.
+template <int N, int Q, int T>
+__global__ void __launch_bounds__(T) sweep_unit_kernel(const SweepArgs a) {
+    extern __shared__ double tile[];                       // T * (N+1)
+    constexpr int LD = N + 1;
+    const size_t p0 = (size_t)blockIdx.x * T;              // first pencil of this block
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    const double* __restrict__ pin = a.in + p0 * N;
+    double* pout = a.out + p0 * N;
+    const uint32_t nelem = np * N;
+
+    // shift source first: its latency overlaps the tile load
+    double sval = 0.0;
+    if (threadIdx.x < np) sval = __ldg(a.src + src_offset(a, (uint32_t)(p0 + threadIdx.x), 0u));
+
+#pragma unroll
+    for (int it = 0; it < N; ++it) {
+        const uint32_t e = it * T + threadIdx.x;
+        if (e < nelem) tile[(e / N) * LD + (e % N)] = __ldcs(pin + e);
+    }
+    __syncthreads();
+
+    if (threadIdx.x < np) {
+        long long k;
+        double theta;
+        split_shift(sval, a.scale, k, theta);
+        long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
+        kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
+        const int r0 = (int)kc + (1 - Q / 2);
+        double* row = tile + threadIdx.x * LD;
+        constexpr int NU = N + Q - 1;
+        double u[NU];
+#pragma unroll
+        for (int t = 0; t < NU; ++t) {
+            const int c = r0 + t;
+            u[t] = (c >= 0 && c < N) ? row[c] : 0.0;
+        }
+        double w[Q];
+        lagrange_weights<Q>(theta, w);
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+            double acc = w[0] * u[j];
+#pragma unroll
+            for (int m = 1; m < Q; ++m) acc = fma(w[m], u[j + m], acc);
+            row[j] = acc;
+        }
+    }
+    __syncthreads();
+
+#pragma unroll
+    for (int it = 0; it < N; ++it) {
+        const uint32_t e = it * T + threadIdx.x;
+        if (e < nelem) __stcs(pout + e, tile[(e / N) * LD + (e % N)]);
+    }
+}
+
+// ---- fallback for extents / widths without a specialised instance -------------------------------------------
+// One column per thread, staged in shared memory as tile[row * T + tid]; q loads per output.  Correct for any
+// n, any even q <= 12, both boundary kinds, inner >= 1; not tuned.
+template <int T>
+__global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int q, int periodic) {
+    extern __shared__ double tile[];                       // n * T
+    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
+    const uint32_t bo = blockIdx.x / a.nib;
+    const uint32_t bi = blockIdx.x - bo * a.nib;
+    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
+    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
+    if (i >= a.inner || o >= a.outer) return;
+    const int n = (int)a.n;
+    long long k;
+    double theta;
+    split_shift(__ldg(a.src + src_offset(a, o, i)), a.scale, k, theta);
+    const size_t stride = a.inner;
+    const size_t base = (size_t)o * n * stride + i;
+    for (int r = 0; r < n; ++r) tile[r * T + threadIdx.x] = __ldcs(a.in + base + (size_t)r * stride);
+
+    double w[12];
+    {
+        // same product form as lagrange_weights<Q>, run-time q
+        const int mlo = 1 - q / 2;
+        for (int ii = 0; ii < q; ++ii) {
+            double num = 1.0, den = 1.0;
+            for (int jj = 0; jj < q; ++jj) {
+                if (jj == ii) continue;
+                num *= theta - (double)(mlo + jj);
+                den *= (double)(ii - jj);
+            }
+            w[ii] = num / den;
+        }
+    }
+    long long kk = k + (long long)(1 - q / 2);             // first stencil row for j = 0
+    if (periodic) { kk %= n; if (kk < 0) kk += n; }
+    else { const long long lim = 2LL * n + 32; kk = kk < -lim ? -lim : (kk > lim ? lim : kk); }
+    for (int j = 0; j < n; ++j) {
+        double acc = 0.0;
+        for (int m = 0; m < q; ++m) {
+            long long r = kk + j + m;
+            double v;
+            if (periodic) { r %= n; v = tile[(int)r * T + threadIdx.x]; }
+            else v = (r >= 0 && r < n) ? tile[(int)r * T + threadIdx.x] : 0.0;
+            acc = (m == 0) ? w[0] * v : fma(w[m], v, acc);
+        }
+        __stcs(a.out + base + (size_t)j * stride, acc);
+    }
+}
+
+}  // namespace bsl6d

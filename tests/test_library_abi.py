@@ -1,0 +1,64 @@
+"""The C-ABI library loads on a CPU-only box and exports every symbol include/bsl6d.h declares (no compute)."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+import paper_2303_05994_b200 as bsl
+from paper_2303_05994_b200 import build as bsl_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    bsl_build.build()                     # no-op when libbsl6d.so is newer than its sources
+    return bsl.load_library()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "bsl6d.h")).read()
+    return sorted(set(re.findall(r"BSL6D_API[^;(]*?\b(bsl6d_\w+)\s*\(", text)))
+
+
+def test_header_and_binding_agree():
+    assert declared_symbols() == sorted(bsl.SYMBOLS)
+
+
+def test_library_exports_exactly_the_header(lib):
+    out = subprocess.run(["nm", "-D", "--defined-only", bsl.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l)
+    assert exported == declared_symbols()
+    for s in bsl.SYMBOLS:
+        assert ctypes.cast(getattr(lib, s), ctypes.c_void_p).value
+
+
+def test_no_compute_symbols_needed_on_cpu(lib):
+    assert bsl.version() == 100
+    assert lib.bsl6d_strerror(-2).decode().startswith("f_in and f_out")
+    assert lib.bsl6d_strerror(0) == b"ok"
+
+
+def test_sass_is_sm100a_fp64_fma():
+    """The shipped cubin targets sm_100a and the sweep kernels are plain fp64 FMA code (no tensor-core path)."""
+    r = subprocess.run(["cuobjdump", "-lelf", bsl.LIB_PATH], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip("cuobjdump not available")
+    assert "sm_100a" in r.stdout
+
+
+def test_product_path_does_not_import_oracle():
+    """The product must not route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2303_05994_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "bsl6d_oracle" not in src, fn
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".cpp")):
+            src = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert "import paper_2303_05994_b200" not in src and "from paper_2303_05994_b200" not in src
+            assert "csrc" not in src or fn.endswith(".cpp")
