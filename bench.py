@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the BSL6D split-advection hot path on B200 (driver contract: one JSON line).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C2]
+
+One *step* = one pass of the whole hot path over the resident distribution function of
+BASELINE.json configs[1] (C2: fp64 32^6, degree 7):
+    six 1-D sweeps x1,x2,x3 (shift v_d*dt/dx_d) and v1,v2,v3 (shift E_d(x)*dt/dv_d), dt = 0.05      [a1-a4]
+    the magnetic rotation as three velocity shears (B along x3, theta = 0.1: configs[3] on the same grid) [a5]
+    the density moment rho(x)                                                                          [a6]
+sequenced on one stream through the C ABI (a7's job).  `value` counts the 9 sweeps' point updates per second
+(the density pass is inside the timed region but adds nothing to the numerator).
+
+Timing: CUDA events on the launching stream, W >= 3 warm-up steps, barrier + synchronize on both sides, max over
+ranks.  Inputs (8.6 GB per buffer) are far larger than the 126 MB L2, so no explicit flush is needed.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+Multi-GPU: the path has no exchange step on one node (replicas only) -- every rank runs
+an independent replica of the workload, `value` is the aggregate, scaling = weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from dataclasses import replace
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "fp64 1-D advection sweep Gpoint-updates/s (16 B/point/sweep), whole hot-path step"
+UNIT = "Gpoint-updates/s"
+ROT_DT = 0.1          # theta = |B| * dt = 0.1 (BASELINE.json configs[3])
+ROT_B = (0.0, 0.0, 1.0)
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=10)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    p.add_argument("--workload", default="C2", help="C1..C5 (C2 = BASELINE configs[1] is the contract workload)")
+    p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    p.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    return p.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.tmp = None
+
+    def start(self):
+        try:
+            self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        try:
+            self.tmp.flush()
+            self.tmp.seek(0)
+            rows = [r.strip().split(",") for r in self.tmp.read().strip().splitlines() if r.strip()]
+            self.tmp.close()
+            os.unlink(self.tmp.name)
+        except Exception:
+            return out
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if r[3 + k].strip().lower().startswith("active"):
+                    reasons.add(nm)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------------------
+# the step, as a list of ops (shared description; the GPU leg and the oracle leg each execute it their own way)
+# ------------------------------------------------------------------------------------------------------------
+def step_ops(w):
+    """[(name, kind, dim)]: the order of one step."""
+    ops = [(nm, "advect", d) for d, nm in enumerate(("x1", "x2", "x3", "v1", "v2", "v3"))]
+    ops.append(("rot", "rotate", -1))
+    ops.append(("rho", "density", -1))
+    return ops
+
+
+N_SWEEPS = 9          # 6 advect + 3 shears
+
+
+# ------------------------------------------------------------------------------------------------------------
+# oracle leg (cpu_baseline and --impl reference): a BOUNDED sample of the same workload on the host cores
+# ------------------------------------------------------------------------------------------------------------
+class OracleSample:
+    """For each op of the step, a crop of the workload's grid (same lo/dx/degree/fields): the swept dim and the
+    three v dims keep their full extent, the other x dims are cropped so that a crop holds <= ~6.7e7 points
+    (crops of equal shape share their buffers)."""
+
+    def __init__(self, w, target_pts=1 << 26):
+        import oracle
+        self.oracle = oracle
+        self.w = w
+        self.cases = []
+        shared = {}
+        nv = int(np.prod(w.n[3:], dtype=np.int64))
+        for name, kind, dim in step_ops(w):
+            n = list(w.n)
+            if kind == "advect" and dim < 3:
+                rest = [d for d in range(3) if d != dim]
+                budget = max(1, target_pts // (nv * w.n[dim]))
+                c = max(1, int(round(budget ** 0.5)))
+                for d in rest:
+                    n[d] = min(w.n[d], c)
+            else:
+                budget = max(1, target_pts // nv)
+                c = max(1, int(round(budget ** (1.0 / 3.0))))
+                for d in range(3):
+                    n[d] = min(w.n[d], c)
+            sub = replace(w, n=tuple(n), name=f"{w.name}_crop_{name}")
+            if tuple(n) not in shared:
+                f = sub.make_f("cpu").numpy()
+                shared[tuple(n)] = (f, np.empty_like(f))
+            f, out = shared[tuple(n)]
+            g = oracle.Grid(tuple(sub.n), tuple(sub.lo), tuple(sub.dx))
+            E = sub.E()
+            self.cases.append((name, kind, dim, sub, g, f, out, E))
+        self.sweep_pts = sum((3 if k == "rotate" else 1) * c[3].npts for c in self.cases for k in [c[1]]
+                             if k != "density")
+        self.desc = "per op a crop of the %s grid: " % w.name + ", ".join(
+            f"{c[0]}:{'x'.join(map(str, c[3].n))}" for c in self.cases)
+
+    def run_once(self):
+        o, w = self.oracle, self.w
+        t0 = time.perf_counter()
+        for name, kind, dim, sub, g, f, out, E in self.cases:
+            if kind == "advect":
+                o.advect(g, sub.degree, f, dim, None if dim < 3 else E[dim - 3], w.dt, out=out)
+            elif kind == "rotate":
+                o.rotate(g, sub.degree, f, ROT_B, ROT_DT, out=out)
+            else:
+                o.density(g, f)
+        return time.perf_counter() - t0
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the host cores.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    samp = OracleSample(w)
+    for _ in range(min(args.warmup, 1)):
+        samp.run_once()
+    t = 0.0
+    for _ in range(args.steps):
+        t += samp.run_once()
+    val = samp.sweep_pts * args.steps / t / 1e9
+    cores = oracle.num_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name} {'x'.join(map(str, w.n))} degree {w.degree}: six sweeps + rotation "
+                               f"shears + density; oracle on a bounded sample", "sample": samp.desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": samp.desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# GPU leg
+# ------------------------------------------------------------------------------------------------------------
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    import paper_2303_05994_b200 as bsl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    bsl.load_library()                                    # fail loudly if the extension is missing
+
+    dev = torch.device("cuda", local)
+    npts = w.npts
+    nx = w.n[0] * w.n[1] * w.n[2]
+    a = w.make_f(dev)                                     # seeded synthetic f (bsl6d_workloads), resident in HBM
+    f0_host = None
+    if not args.no_e2e:
+        f0_host = torch.empty(w.n, dtype=torch.float64, pin_memory=True)
+        f0_host.copy_(a)
+    b = torch.empty_like(a)
+    rho = torch.empty(w.n[:3], dtype=torch.float64, device=dev)
+    E_host = [torch.from_numpy(e) for e in w.E()]
+    E = [e.to(dev) for e in E_host]
+    ctx = bsl.create(w.n, w.lo, w.dx, w.degree)
+    ops = step_ops(w)
+    kernels = {nm: (ctx.kernel_name(d) if kind == "advect" else "") for nm, kind, d in ops}
+    kernels["rot"] = f"{ctx.kernel_name(3)} + {ctx.kernel_name(4)} + {ctx.kernel_name(3)}"
+    stream = torch.cuda.current_stream()
+
+    def one_step(cur, oth, evs=None):
+        for i, (name, kind, dim) in enumerate(ops):
+            if evs is not None:
+                evs[i].record(stream)
+            if kind == "advect":
+                ctx.advect(cur, oth, dim, None if dim < 3 else E[dim - 3], w.dt)
+                cur, oth = oth, cur
+            elif kind == "rotate":
+                ctx.rotate(cur, oth, ROT_B, ROT_DT)
+                cur, oth = oth, cur
+            else:
+                ctx.density(cur, rho)
+        if evs is not None:
+            evs[len(ops)].record(stream)
+        return cur, oth
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cur, oth = a, b
+    for _ in range(max(args.warmup, 0)):
+        cur, oth = one_step(cur, oth)
+    barrier()
+
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(ops) + 1)] for _ in range(K)]
+    l0 = ctx.launch_count()
+    clocks = ClockSampler(local)
+    clocks.start()
+    time.sleep(0.25)
+    barrier()
+    t_wall = time.perf_counter()
+    for s in range(K):
+        cur, oth = one_step(cur, oth, evs[s])
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    # keep the sampler alive for a moment if the region was very short, so that it has samples under load
+    clk = clocks.stop()
+    launches = ctx.launch_count() - l0
+    total_ms = evs[0][0].elapsed_time(evs[K - 1][len(ops)])
+    per_op = {nm: float(np.mean([evs[s][i].elapsed_time(evs[s][i + 1]) for s in range(K)]))
+              for i, (nm, _, _) in enumerate(ops)}
+    assert torch.isfinite(rho).all()
+
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+
+    value = world * N_SWEEPS * npts * K / (total_ms * 1e-3) / 1e9
+    step_bytes = (N_SWEEPS * 16 * npts + 8 * npts + 8 * nx)
+
+    # ---- roofline of the dominant kernel: the strided sweep (x1,x2,x3,v1,v2 + the three shears = 8 launches/step)
+    peak, peak_src = peaks()
+    strided_ms = sum(per_op[nm] for nm in ("x1", "x2", "x3", "v1", "v2", "rot")) / 8.0
+    achieved = 16.0 * npts / (strided_ms * 1e-3) / 1e9
+    per_dim = {}
+    for nm, kind, _ in ops:
+        nl = 3 if kind == "rotate" else 1
+        bytes_ = (8 * npts + 8 * nx) if kind == "density" else 16 * npts * nl
+        gbs = bytes_ / (per_op[nm] * 1e-3) / 1e9
+        per_dim[nm] = {"ms": per_op[nm], "GB/s": gbs, "frac_of_measured_peak": gbs / peak,
+                       "frac_of_8TBs": gbs / 8000.0, "kernel": kernels.get(nm, "")}
+        if kind != "density":
+            per_dim[nm]["Gpoint-updates/s"] = nl * npts / (per_op[nm] * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")        # written by hand from an `ncu --set full` capture
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(w.name, {}).get("strided_sweep_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": "sweep_strided_kernel (8 of 10 launches per step)", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": 16 * npts, "avg_launch_ms": strided_ms,
+                "step_GB/s": step_bytes / (total_ms / K * 1e-3) / 1e9,
+                "step_frac": step_bytes / (total_ms / K * 1e-3) / 1e9 / peak}
+
+    # ---- e2e: the same step through bsl6d_run_host on HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        del a, b, cur, oth
+        torch.cuda.empty_cache()
+        hops = []
+        for name, kind, dim in ops:
+            if kind == "advect":
+                hops.append({"kind": "advect", "dim": dim, "dt": w.dt,
+                             "shift_source": None if dim < 3 else E_host[dim - 3]})
+            elif kind == "rotate":
+                hops.append({"kind": "rotate", "B": ROT_B, "dt": ROT_DT})
+            else:
+                hops.append({"kind": "density", "rho_host": torch.empty(w.n[:3], dtype=torch.float64,
+                                                                           pin_memory=True)})
+        ke = max(1, min(K, 5))
+        ctx.run_host(f0_host, f0_host, hops)              # warm-up (allocates the context's device buffer)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            ctx.run_host(f0_host, f0_host, hops)
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([te], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            te = float(t.item())
+        e2e = {"value": world * N_SWEEPS * npts * ke / te / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 8 * npts + 3 * 8 * nx, "d2h_bytes_per_step": 8 * npts + 8 * nx,
+               "steps": ke, "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (pinned host buffers)"}
+    ctx.destroy()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        import oracle
+        oracle.build()
+        samp = OracleSample(w)
+        npass = 3
+        tc = sum(samp.run_once() for _ in range(npass))
+        cpu = {"value": npass * samp.sweep_pts / tc / 1e9, "passes": npass, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": samp.desc, "seconds": tc}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name} (BASELINE configs[1]) fp64 {'x'.join(map(str, w.n))}, degree "
+                                   f"{w.degree}: sweeps x1,x2,x3,v1,v2,v3 (dt={w.dt}) + rotation shears v1,v2,v1 "
+                                   f"(theta={ROT_DT}) + density, per replica",
+                       "l2": "inputs (8.6 GB per buffer) larger than the 126 MB L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "wall_ms_per_step": 1e3 * t_wall / K},
+            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu, "per_dim": per_dim,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    import bsl6d_workloads as wl
+    w = wl.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()
