@@ -41,22 +41,47 @@ struct KernelChoice {
     int threads;
     size_t smem;
     int kind;                 // 0 strided, 1 unit, 2 generic
-    int gen_T;
+    int gen_T;                // generic: threads; unit: segments per pencil S
 };
 
+// Launch shape of the strided sweep: T threads per block, at least MINB resident blocks per SM (caps the
+// registers ptxas may use: a thread holds its whole pencil, 2*(N [+Q-1]) registers, plus 2*Q for the weights).
+#ifdef BSL6D_TUNE_T
+template <int N, int Q, bool P> constexpr int strided_threads() { return BSL6D_TUNE_T; }
+template <int N, int Q, bool P> constexpr int strided_minblocks() { return BSL6D_TUNE_MINB; }
+#else
 template <int N, int Q, bool P>
-constexpr int strided_threads() { return N <= 32 ? 256 : 128; }
+constexpr int strided_threads() { return 128; }
+template <int N, int Q, bool P>
+constexpr int strided_minblocks() {
+    constexpr int est = 2 * (N + (P ? 0 : Q - 1)) + 2 * Q + 24;      // registers a thread wants
+    return est <= 128 ? 4 : (est <= 176 ? 3 : 2);
+}
+#endif
 
 template <int N, int Q, bool P>
 KernelChoice strided_choice() {
     constexpr int T = strided_threads<N, Q, P>();
-    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T>, T, 0, 0, 0};
+    constexpr int MINB = strided_minblocks<N, Q, P>();
+    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB>, T, 0, 0, 0};
 }
+
+// Launch shape of the unit-stride sweep: S segments per pencil, T threads (a multiple of 32*S), MINB blocks/SM.
+#ifdef BSL6D_TUNE_US
+template <int N, int Q> constexpr int unit_segments() { return (N % BSL6D_TUNE_US == 0) ? BSL6D_TUNE_US : 1; }
+template <int N, int Q> constexpr int unit_minblocks() { return BSL6D_TUNE_UMINB; }
+#else
+template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 2 : 1; }
+template <int N, int Q> constexpr int unit_minblocks() { return 3; }
+#endif
+template <int N, int Q> constexpr int unit_threads() { return 128 % (32 * unit_segments<N, Q>()) == 0 ? 128 : 32 * unit_segments<N, Q>(); }
 
 template <int N, int Q>
 KernelChoice unit_choice() {
-    constexpr int T = 128;
-    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, T>, T, sizeof(double) * T * (N + 1), 1, 0};
+    constexpr int S = unit_segments<N, Q>();
+    constexpr int T = unit_threads<N, Q>();
+    constexpr int MINB = unit_minblocks<N, Q>();
+    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N + 1), 1, S};
 }
 
 template <int N, bool P>
@@ -199,7 +224,8 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     // ---- grid -------------------------------------------------------------------------------------------
     unsigned grid;
     if (kc.kind == 1) {
-        grid = (unsigned)((outer + kc.threads - 1) / kc.threads);
+        const size_t pb = (size_t)kc.threads / (size_t)kc.gen_T;      // pencils per block = T / S
+        grid = (unsigned)((outer + pb - 1) / pb);
     } else {
         const uint64_t lim = inner < (uint64_t)kc.threads ? inner : (uint64_t)kc.threads;
         a.ti_log2 = ceil_pow2_log2(lim);
@@ -354,8 +380,11 @@ int bsl6d_kernel_name(const bsl6d_ctx* c, int dim, char* buf, int buflen) {
     int rc = choose_kernel(c, dim, k);
     if (rc) return rc;
     const char* kind = k.kind == 0 ? "strided" : (k.kind == 1 ? "unit" : "generic");
-    std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
-                  dim < 3 ? "periodic" : "zero", k.threads);
+    if (k.kind == 1)
+        std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q, k.gen_T, k.threads);
+    else
+        std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
+                      dim < 3 ? "periodic" : "zero", k.threads);
     return BSL6D_OK;
 }
 

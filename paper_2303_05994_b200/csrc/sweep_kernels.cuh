@@ -100,8 +100,8 @@ __device__ __forceinline__ uint32_t src_offset(const SweepArgs& a, uint32_t o, u
 }
 
 // ---- a4: strided sweep, one column per thread, no shared memory --------------------------------------------
-template <int N, int Q, bool PERIODIC, int T>
-__global__ void __launch_bounds__(T) sweep_strided_kernel(const SweepArgs a) {
+template <int N, int Q, bool PERIODIC, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs a) {
     const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
     const uint32_t bo = blockIdx.x / a.nib;
     const uint32_t bi = blockIdx.x - bo * a.nib;
@@ -154,39 +154,53 @@ __global__ void __launch_bounds__(T) sweep_strided_kernel(const SweepArgs a) {
 }
 
 // ---- a3: unit-stride sweep (swept dim is the contiguous one; always a v dim => zero extension) -------------
-// A block owns T consecutive pencils = one contiguous chunk of T*N doubles.  Coalesced load -> padded smem
-// (row stride N+1 doubles: conflict-free for "lane = pencil" access) -> each thread reads ITS pencil in shifted
-// order into registers -> results back into the same smem row -> coalesced store.
-template <int N, int Q, int T>
-__global__ void __launch_bounds__(T) sweep_unit_kernel(const SweepArgs a) {
-    extern __shared__ double tile[];                       // T * (N+1)
+// A block owns PB = T/S consecutive pencils = one contiguous chunk of PB*N doubles.  Coalesced load -> padded
+// smem (row stride N+1 doubles: conflict-free for "lane = pencil" access).  A pencil is cut into S segments of
+// R = N/S outputs; thread (pencil p, segment s) reads the R+Q-1 inputs of its segment in shifted order into
+// registers (all lanes of a warp share s, so every smem access of a warp is conflict-free), forms its R outputs,
+// and after a barrier writes them back into the same smem row -> coalesced store.  S > 1 keeps the register
+// window small for long pencils (N = 48, 64) so that >= 3-4 blocks stay resident per SM and overlap their
+// load / compute / store phases.
+template <int N, int Q, int S, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB) sweep_unit_kernel(const SweepArgs a) {
+    static_assert(N % S == 0 && T % (32 * S) == 0, "segments must tile the pencil and the block");
+    extern __shared__ double tile[];                       // PB * (N+1)
     constexpr int LD = N + 1;
-    const size_t p0 = (size_t)blockIdx.x * T;              // first pencil of this block
-    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    constexpr int PB = T / S;                              // pencils per block
+    constexpr int R = N / S;                               // outputs per thread
+    constexpr int NE = PB * N;                             // elements per full block
+    const size_t p0 = (size_t)blockIdx.x * PB;             // first pencil of this block
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)PB ? ((size_t)a.outer - p0) : (size_t)PB);
     const double* __restrict__ pin = a.in + p0 * N;
     double* pout = a.out + p0 * N;
     const uint32_t nelem = np * N;
 
+    // thread -> (pencil, segment): warp w serves segment w % S of pencils 32*(w/S) .. 32*(w/S)+31
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t seg = warp % S;
+    const uint32_t pl = (warp / S) * 32u + lane;           // pencil within the block
+
     // shift source first: its latency overlaps the tile load
     double sval = 0.0;
-    if (threadIdx.x < np) sval = __ldg(a.src + src_offset(a, (uint32_t)(p0 + threadIdx.x), 0u));
+    if (pl < np) sval = __ldg(a.src + src_offset(a, (uint32_t)(p0 + pl), 0u));
 
 #pragma unroll
-    for (int it = 0; it < N; ++it) {
+    for (int it = 0; it < (NE + T - 1) / T; ++it) {
         const uint32_t e = it * T + threadIdx.x;
         if (e < nelem) tile[(e / N) * LD + (e % N)] = __ldcs(pin + e);
     }
     __syncthreads();
 
-    if (threadIdx.x < np) {
+    double res[R];
+    if (pl < np) {
         long long k;
         double theta;
         split_shift(sval, a.scale, k, theta);
         long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
         kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
-        const int r0 = (int)kc + (1 - Q / 2);
-        double* row = tile + threadIdx.x * LD;
-        constexpr int NU = N + Q - 1;
+        const int r0 = (int)kc + (1 - Q / 2) + (int)seg * R;
+        const double* row = tile + pl * LD;
+        constexpr int NU = R + Q - 1;
         double u[NU];
 #pragma unroll
         for (int t = 0; t < NU; ++t) {
@@ -196,17 +210,23 @@ __global__ void __launch_bounds__(T) sweep_unit_kernel(const SweepArgs a) {
         double w[Q];
         lagrange_weights<Q>(theta, w);
 #pragma unroll
-        for (int j = 0; j < N; ++j) {
+        for (int j = 0; j < R; ++j) {
             double acc = w[0] * u[j];
 #pragma unroll
             for (int m = 1; m < Q; ++m) acc = fma(w[m], u[j + m], acc);
-            row[j] = acc;
+            res[j] = acc;
         }
+    }
+    if (S > 1) __syncthreads();                            // other segments of my row may still be reading it
+    if (pl < np) {
+        double* row = tile + pl * LD + seg * R;
+#pragma unroll
+        for (int j = 0; j < R; ++j) row[j] = res[j];
     }
     __syncthreads();
 
 #pragma unroll
-    for (int it = 0; it < N; ++it) {
+    for (int it = 0; it < (NE + T - 1) / T; ++it) {
         const uint32_t e = it * T + threadIdx.x;
         if (e < nelem) __stcs(pout + e, tile[(e / N) * LD + (e % N)]);
     }

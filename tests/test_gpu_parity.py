@@ -352,7 +352,7 @@ def test_error_codes():
             ctx.advect(a, a, 3, None, 0.1)                    # E sweep needs a source
         assert e.value.code == bsl.EINVAL
         with pytest.raises(bsl.Bsl6dError) as e:
-            ctx.advect_generic(a, a, 2, a, 1 << 2, 1.0)       # mask contains the swept dim
+            ctx.advect_generic(a, a, 2, a[:w.n[2]], 1 << 2, 1.0)   # mask contains the swept dim
         assert e.value.code == bsl.EINVAL
         with pytest.raises(bsl.Bsl6dError) as e:
             ctx.advect(a, a, 0, None, float("nan"))
