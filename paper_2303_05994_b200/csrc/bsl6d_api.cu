@@ -71,8 +71,8 @@ KernelChoice strided_choice() {
 template <int N, int Q> constexpr int unit_segments() { return (N % BSL6D_TUNE_US == 0) ? BSL6D_TUNE_US : 1; }
 template <int N, int Q> constexpr int unit_minblocks() { return BSL6D_TUNE_UMINB; }
 #else
-template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 2 : 1; }
-template <int N, int Q> constexpr int unit_minblocks() { return 3; }
+template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 4 : 1; }
+template <int N, int Q> constexpr int unit_minblocks() { return 4; }
 #endif
 template <int N, int Q> constexpr int unit_threads() { return 128 % (32 * unit_segments<N, Q>()) == 0 ? 128 : 32 * unit_segments<N, Q>(); }
 
