@@ -318,11 +318,14 @@ def run_ours(args, w):
         if kind != "density":
             per_dim[nm]["Gpoint-updates/s"] = nl * npts / (per_op[nm] * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")        # written by hand from an `ncu --set full` capture
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")         # copied from an `ncu --set full` capture (traffic.md)
     if os.path.exists(tpath):
         try:
             with open(tpath) as fh:
-                traffic = json.load(fh).get(w.name, {}).get("strided_sweep_bytes_per_launch")
+                for ln in fh.read().splitlines()[1:]:
+                    c = ln.split(",")
+                    if c[0] == w.name and c[1] == "sweep_strided_kernel":
+                        traffic = float(c[2])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": "sweep_strided_kernel (8 of 10 launches per step)", "achieved": achieved,
