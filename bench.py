@@ -134,6 +134,25 @@ N_SWEEPS = 9          # 6 advect + 3 shears
 
 
 # ------------------------------------------------------------------------------------------------------------
+# multi-rank host logic (replicas only: no data-path collective; covered by a world_size-2 gloo test on CPU)
+# ------------------------------------------------------------------------------------------------------------
+def max_over_ranks(x: float, device=None) -> float:
+    """MAX of a per-rank scalar over the process group (identity without one)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(npts: int, n_sweeps: int, steps: int, world: int, total_ms: float) -> float:
+    """Gpoint-updates/s of the whole job: every rank advanced its own replica; time = max over ranks."""
+    return world * n_sweeps * npts * steps / (total_ms * 1e-3) / 1e9
+
+
+# ------------------------------------------------------------------------------------------------------------
 # oracle leg (cpu_baseline and --impl reference): a BOUNDED sample of the same workload on the host cores
 # ------------------------------------------------------------------------------------------------------------
 class OracleSample:
@@ -296,12 +315,8 @@ def run_ours(args, w):
               for i, (nm, _, _) in enumerate(ops)}
     assert torch.isfinite(rho).all()
 
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-
-    value = world * N_SWEEPS * npts * K / (total_ms * 1e-3) / 1e9
+    total_ms = max_over_ranks(total_ms, dev)
+    value = whole_job_value(npts, N_SWEEPS, K, world, total_ms)
     step_bytes = (N_SWEEPS * 16 * npts + 8 * npts + 8 * nx)
 
     # ---- roofline of the dominant kernel: the strided sweep (x1,x2,x3,v1,v2 + the three shears = 8 launches/step)
@@ -357,11 +372,8 @@ def run_ours(args, w):
             ctx.run_host(f0_host, f0_host, hops)
         torch.cuda.synchronize()
         te = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([te], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
-        e2e = {"value": world * N_SWEEPS * npts * ke / te / 1e9, "unit": UNIT,
+        te = max_over_ranks(te, dev)
+        e2e = {"value": whole_job_value(npts, N_SWEEPS, ke, world, 1e3 * te), "unit": UNIT,
                "h2d_bytes_per_step": 8 * npts + 3 * 8 * nx, "d2h_bytes_per_step": 8 * npts + 8 * nx,
                "steps": ke, "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (pinned host buffers)"}
     ctx.destroy()
