@@ -85,7 +85,8 @@ BSL6D_API int bsl6d_advect_generic(bsl6d_ctx* ctx, const double* f_in, double* f
  * shears (BASELINE.json configs[3], reading S7): with B (HOST, 3 doubles, = (q/m)*B0) along axis c,
  * (a,b,c) cyclic, theta = B[c]*dt:  shear v_a by foot displacement -v_b*tan(theta/2), shear v_b by
  * +v_a*sin(theta), shear v_a again.  Result: f_out(v) = f_in(R(theta) v).  Exactly one component of B may be
- * non-zero (else BSL6D_EUNSUPPORTED); B == 0 copies f_in to f_out.  Three sweeps: f_in -> f_out, then in place. */
+ * non-zero (else BSL6D_EUNSUPPORTED); B == 0 copies f_in to f_out.  One fused pass f_in -> f_out where a fused kernel
+ * exists (B along x3 on the specialised extents), else three sweeps: f_in -> f_out, then in place. */
 BSL6D_API int bsl6d_rotate(bsl6d_ctx* ctx, const double* f_in, double* f_out, const double B[3], double dt, void* stream);
 
 /* One Strang-split time step (order per BASELINE.json configs[4], reading S8), result in f:
@@ -95,6 +96,30 @@ BSL6D_API int bsl6d_rotate(bsl6d_ctx* ctx, const double* f_in, double* f_out, co
  * if given the sweeps ping-pong between f and f_tmp, if NULL they run in place.  The numbers are identical. */
 BSL6D_API int bsl6d_strang_step(bsl6d_ctx* ctx, double* f, double* f_tmp, const double* const E[3], const double B[3],
                       double dt, void* stream);
+
+/* ---- sequences of sweeps, fused on chip ------------------------------------------------
+ * The Lie-split step is a chain of 1-D sweeps.  Wherever consecutive sweeps of a chain act along
+ * only two dims a < b (b not the unit-stride dim) -- x1 then x2, x3 then v1, the three shears v_a, v_b, v_a of a
+ * rotation -- the library stages tiles [n_a][n_b][C contiguous doubles] in shared memory and applies the two or
+ * three sweeps in ONE pass over f: 16 B/point of HBM traffic per pass instead of per sweep.  Per sweep the
+ * arithmetic is unchanged, so the numbers are bit-identical to issuing the sweeps one by one.
+ * bsl6d_rotate, bsl6d_strang_step and bsl6d_advect_seq all go through this planner; a group without a fused
+ * kernel (extent not in {8,16,32,48,64}, degree not in {5,7,9}, inner extent not a multiple of C) silently runs
+ * as single sweeps.  bsl6d_set_fusion(ctx, 0) turns grouping off (every sweep its own pass); returns the old
+ * setting (default 1). */
+typedef struct bsl6d_sweep {
+    int32_t dim;             /* swept dim 0..5 */
+    uint32_t src_dim_mask;   /* dims the shift source is dense over (bit d), must not contain `dim` */
+    const double* src;       /* DEVICE; NULL with dim < 3 selects the grid's v_dim nodes (mask is then ignored) */
+    double scale;            /* alpha_cells = -(src[p] * scale), as in bsl6d_advect_generic */
+} bsl6d_sweep;
+/* Apply sweeps[0..nsweeps) in order: the first pass reads f_in and writes f_out, later passes run in place on
+ * f_out (f_in == f_out is legal).  nsweeps <= 64; nsweeps == 0 copies. */
+BSL6D_API int bsl6d_advect_seq(bsl6d_ctx* ctx, const double* f_in, double* f_out, const bsl6d_sweep* sweeps,
+                     int nsweeps, void* stream);
+/* Number of passes (kernel launches) bsl6d_advect_seq would use for this chain, or a negative error code. */
+BSL6D_API int bsl6d_seq_passes(bsl6d_ctx* ctx, const bsl6d_sweep* sweeps, int nsweeps);
+BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
 
 /* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */

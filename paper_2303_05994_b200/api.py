@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libbsl6d.so")
 SYMBOLS = (
     "bsl6d_create", "bsl6d_destroy", "bsl6d_advect", "bsl6d_advect_generic", "bsl6d_rotate",
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
-    "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version",
+    "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
+    "bsl6d_set_fusion",
 )
 
 OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
@@ -33,6 +34,11 @@ class HostOp(C.Structure):
     """bsl6d_host_op."""
     _fields_ = [("kind", C.c_int32), ("dim", C.c_int32), ("shift_source", C.c_void_p), ("dt", C.c_double),
                 ("B", C.c_double * 3), ("rho_host", C.c_void_p)]
+
+
+class Sweep(C.Structure):
+    """bsl6d_sweep."""
+    _fields_ = [("dim", C.c_int32), ("src_dim_mask", C.c_uint32), ("src", C.c_void_p), ("scale", C.c_double)]
 
 
 class Bsl6dError(RuntimeError):
@@ -70,6 +76,9 @@ def load_library() -> C.CDLL:
     lib.bsl6d_launch_count.restype = C.c_longlong
     lib.bsl6d_kernel_name.argtypes = [vp, C.c_int, C.c_char_p, C.c_int]
     lib.bsl6d_version.restype = C.c_int
+    lib.bsl6d_advect_seq.argtypes = [vp, dp, dp, C.POINTER(Sweep), C.c_int, vp]
+    lib.bsl6d_seq_passes.argtypes = [vp, C.POINTER(Sweep), C.c_int]
+    lib.bsl6d_set_fusion.argtypes = [vp, C.c_int]
     _lib = lib
     return lib
 
@@ -178,6 +187,33 @@ class Context:
         self._check(self._lib.bsl6d_strang_step(self._h, _dev_ptr(f, "f"), _dev_ptr(f_tmp, "f_tmp"), Ep, Bc, float(dt),
                                                 _stream(stream)), "bsl6d_strang_step")
         return f
+
+    def _sweeps(self, sweeps):
+        """sweeps: (dim, src tensor or None, src_dim_mask, scale) tuples -> bsl6d_sweep array."""
+        arr = (Sweep * max(1, len(sweeps)))()
+        for i, (dim, src, mask, scale) in enumerate(sweeps):
+            arr[i].dim, arr[i].src_dim_mask, arr[i].scale = int(dim), int(mask), float(scale)
+            arr[i].src = _dev_ptr(src, "src")
+        return arr
+
+    def advect_seq(self, f_in, f_out, sweeps, stream=None):
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        arr = self._sweeps(sweeps)
+        self._check(self._lib.bsl6d_advect_seq(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"), arr,
+                                               len(sweeps), _stream(stream)), "bsl6d_advect_seq")
+        return f_out
+
+    def seq_passes(self, sweeps) -> int:
+        rc = self._lib.bsl6d_seq_passes(self._h, self._sweeps(sweeps), len(sweeps))
+        if rc < 0:
+            self._check(rc, "bsl6d_seq_passes")
+        return rc
+
+    def set_fusion(self, enable: bool) -> bool:
+        rc = self._lib.bsl6d_set_fusion(self._h, 1 if enable else 0)
+        if rc < 0:
+            self._check(rc, "bsl6d_set_fusion")
+        return bool(rc)
 
     def density(self, f, rho, stream=None):
         self._shape_ok(f, "f")

@@ -9,6 +9,8 @@
 #include <vector>
 
 #include "density_kernels.cuh"
+#include "fused_api.h"
+#include "fused_kernels.cuh"
 #include "sweep_kernels.cuh"
 
 using bsl6d::SweepArgs;
@@ -25,6 +27,9 @@ struct bsl6d_ctx {
     size_t dens_chunk;
     int last_cuda;
     long long launches;
+    int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
+    const void* smem_ok[16];  // fused kernels whose dynamic shared-memory limit has been raised
+    int n_smem_ok;
     // host-path working set (bsl6d_run_host), allocated on first use
     double* h_f;              // device buffer for f
     double* h_small;          // device buffer for shift sources / rho
@@ -160,6 +165,40 @@ uint32_t ceil_pow2_log2(uint64_t v) {
     return l;
 }
 
+// Source-index terms of a sweep along `dim` whose shift source is dense over the dims in `mask`:
+// runs of adjacent masked dims inside the outer / inner group of the [outer][N][inner] view.
+int build_src_terms(const int32_t* n, int dim, unsigned mask, bsl6d::SrcTerms& t) {
+    std::memset(&t, 0, sizeof(t));
+    size_t sstride[6];
+    {
+        size_t s = 1;
+        for (int d = 5; d >= 0; --d) {
+            if (mask & (1u << d)) { sstride[d] = s; s *= (size_t)n[d]; } else sstride[d] = 0;
+        }
+        if (s > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
+    }
+    for (int grp = 0; grp < 2; ++grp) {
+        const int dlo = grp == 0 ? 0 : dim + 1, dhi = grp == 0 ? dim : 6;   // [dlo, dhi)
+        int d = dhi - 1;
+        size_t below = 1;
+        while (d >= dlo) {
+            if (!(mask & (1u << d))) { below *= (size_t)n[d]; --d; continue; }
+            // run of masked dims d, d-1, ... (towards slower dims)
+            size_t extent = 1;
+            const size_t run_below = below, run_sstride = sstride[d];
+            while (d >= dlo && (mask & (1u << d))) { extent *= (size_t)n[d]; below *= (size_t)n[d]; --d; }
+            const bool slowest = (d < dlo);
+            if (t.nterms >= (uint32_t)bsl6d::kMaxSrcTerms) return BSL6D_EUNSUPPORTED;
+            const uint32_t k = t.nterms++;
+            t.t_inner[k] = (uint32_t)grp;
+            t.t_below[k] = (uint32_t)run_below;
+            t.t_extent[k] = slowest ? 0u : (uint32_t)extent;
+            t.t_sstride[k] = (uint32_t)run_sstride;
+        }
+    }
+    return BSL6D_OK;
+}
+
 // Build the launch arguments and enqueue one sweep.
 int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const double* src, unsigned mask,
                  double scale, cudaStream_t stream) {
@@ -192,34 +231,8 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     a.outer = (uint32_t)outer;
     a.n = (uint32_t)n[dim];
 
-    // ---- source-index terms: runs of adjacent masked dims inside the outer / inner group ----------------
-    size_t sstride[6];
-    {
-        size_t s = 1;
-        for (int d = 5; d >= 0; --d) {
-            if (mask & (1u << d)) { sstride[d] = s; s *= (size_t)n[d]; } else sstride[d] = 0;
-        }
-        if (s > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
-    }
-    for (int grp = 0; grp < 2; ++grp) {
-        const int dlo = grp == 0 ? 0 : dim + 1, dhi = grp == 0 ? dim : 6;   // [dlo, dhi)
-        int d = dhi - 1;
-        size_t below = 1;
-        while (d >= dlo) {
-            if (!(mask & (1u << d))) { below *= (size_t)n[d]; --d; continue; }
-            // run of masked dims d, d-1, ... (towards slower dims)
-            size_t extent = 1;
-            const size_t run_below = below, run_sstride = sstride[d];
-            while (d >= dlo && (mask & (1u << d))) { extent *= (size_t)n[d]; below *= (size_t)n[d]; --d; }
-            const bool slowest = (d < dlo);
-            if (a.nterms >= (uint32_t)bsl6d::kMaxSrcTerms) return BSL6D_EUNSUPPORTED;
-            const uint32_t t = a.nterms++;
-            a.t_inner[t] = (uint32_t)grp;
-            a.t_below[t] = (uint32_t)run_below;
-            a.t_extent[t] = slowest ? 0u : (uint32_t)extent;
-            a.t_sstride[t] = (uint32_t)run_sstride;
-        }
-    }
+    rc = build_src_terms(n, dim, mask, a.terms);
+    if (rc) return rc;
 
     // ---- grid -------------------------------------------------------------------------------------------
     unsigned grid;
@@ -261,6 +274,177 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->launches += 1;
+    return BSL6D_OK;
+}
+
+// ---- sequences of sweeps: planning into passes ---------------------------------------------
+struct SweepDesc { int dim; const double* src; unsigned mask; double scale; };
+
+struct Pass {
+    int first, count;         // sweeps [first, first+count)
+    bool fused;
+    bsl6d::FusedChoice fc;
+    int pattern;
+};
+
+bool fused_lookup(int q, int na, int nb, bool pa, bool pb, int pattern, bsl6d::FusedChoice& fc) {
+    switch (q) {
+        case 6: return bsl6d::fused_lookup_q6(na, nb, pa, pb, pattern, fc);
+        case 8: return bsl6d::fused_lookup_q8(na, nb, pa, pb, pattern, fc);
+        case 10: return bsl6d::fused_lookup_q10(na, nb, pa, pb, pattern, fc);
+        default: return false;
+    }
+}
+
+int check_sweep_desc(const bsl6d_ctx* c, const SweepDesc& s) {
+    if (!s.src) return BSL6D_EINVAL;
+    if (s.dim < 0 || s.dim > 5 || (s.mask & ~0x3Fu) || (s.mask & (1u << s.dim))) return BSL6D_EINVAL;
+    if (!std::isfinite(s.scale)) return BSL6D_EINVAL;
+    (void)c;
+    return BSL6D_OK;
+}
+
+// Can sweeps [i, i+cnt) run as one fused pass?  cnt = 2: dims (a, b); cnt = 3: dims (a, b, a); a < b, b not unit-stride.
+bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) {
+    const int a = sw[i].dim, b = sw[i + 1].dim;
+    if (!(a < b)) return false;
+    if (cnt == 3 && sw[i + 2].dim != a) return false;
+    const int32_t* n = c->g.n;
+    size_t inner_b = 1, mid = 1, outer = 1;
+    for (int d = b + 1; d < 6; ++d) inner_b *= (size_t)n[d];
+    for (int d = a + 1; d < b; ++d) mid *= (size_t)n[d];
+    for (int d = 0; d < a; ++d) outer *= (size_t)n[d];
+    if (inner_b < 2) return false;
+    const int pattern = cnt == 2 ? bsl6d::kPatAB : bsl6d::kPatABA;
+    bsl6d::FusedChoice fc;
+    if (!fused_lookup(c->q, n[a], n[b], a < 3, b < 3, pattern, fc)) return false;
+    if (inner_b % (size_t)fc.C) return false;
+    if (c->npts > 0xFFFFFFFFull) return false;                        // 32-bit pencil indices in the kernel
+    const size_t blocks = outer * mid * (inner_b / (size_t)fc.C);
+    if (blocks > 0x7FFFFFFFull) return false;
+    p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern;
+    return true;
+}
+
+int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pass>& passes) {
+    passes.clear();
+    for (int i = 0; i < ns; ++i) {
+        int rc = check_sweep_desc(c, sw[i]);
+        if (rc) return rc;
+        KernelChoice kc;
+        rc = choose_kernel(c, sw[i].dim, kc);
+        if (rc) return rc;
+    }
+    int i = 0;
+    while (i < ns) {
+        Pass p{i, 1, false, {}, 0};
+        if (c->fusion) {
+            if (!(i + 2 < ns && try_fuse(c, sw, i, 3, p)))
+                if (i + 1 < ns) (void)try_fuse(c, sw, i, 2, p);
+        }
+        passes.push_back(p);
+        i += p.count;
+    }
+    return BSL6D_OK;
+}
+
+int launch_fused(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDesc* sw, const Pass& p,
+                 cudaStream_t stream) {
+    const int a = sw[p.first].dim, b = sw[p.first + 1].dim;
+    const int32_t* n = c->g.n;
+    size_t inner_b = 1, mid = 1, outer = 1;
+    for (int d = b + 1; d < 6; ++d) inner_b *= (size_t)n[d];
+    for (int d = a + 1; d < b; ++d) mid *= (size_t)n[d];
+    for (int d = 0; d < a; ++d) outer *= (size_t)n[d];
+    bsl6d::FusedArgs fa;
+    std::memset(&fa, 0, sizeof(fa));
+    fa.in = f_in;
+    fa.out = f_out;
+    fa.mid = (uint32_t)mid;
+    fa.inner_b = (uint32_t)inner_b;
+    fa.nchunks = (uint32_t)(inner_b / (size_t)p.fc.C);
+    for (int k = 0; k < p.count; ++k) {
+        const SweepDesc& s = sw[p.first + k];
+        fa.sw[k].src = s.src;
+        fa.sw[k].scale = s.scale;
+        int rc = build_src_terms(n, s.dim, s.mask, fa.sw[k].terms);
+        if (rc) return rc;
+    }
+    cudaError_t e;
+    if (p.fc.smem > 48 * 1024) {
+        bool known = false;
+        for (int k = 0; k < c->n_smem_ok; ++k) known = known || c->smem_ok[k] == p.fc.fn;
+        if (!known) {
+            e = cudaFuncSetAttribute(p.fc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.fc.smem);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+            if (c->n_smem_ok < 16) c->smem_ok[c->n_smem_ok++] = p.fc.fn;
+        }
+    }
+    const unsigned grid = (unsigned)(outer * mid * (size_t)fa.nchunks);
+    void* args[] = {(void*)&fa};
+    e = cudaLaunchKernel(p.fc.fn, dim3(grid), dim3(p.fc.threads), args, p.fc.smem, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
+}
+
+int launch_pass(bsl6d_ctx* c, const double* src, double* dst, const SweepDesc* sw, const Pass& p, cudaStream_t st) {
+    if (p.fused) return launch_fused(c, src, dst, sw, p, st);
+    const SweepDesc& s = sw[p.first];
+    return launch_sweep(c, src, dst, s.dim, s.src, s.mask, s.scale, st);
+}
+
+bool partial_overlap(const bsl6d_ctx* c, const void* x, const void* y) {
+    if (x == y) return false;
+    const size_t bytes = c->npts * sizeof(double);
+    const char* a = (const char*)x;
+    const char* b = (const char*)y;
+    return a < b + bytes && b < a + bytes;
+}
+
+// f_in -> f_out: the first pass reads f_in and writes f_out, the others run in place on f_out.
+int run_sequence_in_out(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDesc* sw, int ns,
+                        cudaStream_t st) {
+    if (!c || !f_in || !f_out || ns < 0 || (ns > 0 && !sw)) return BSL6D_EINVAL;
+    if (partial_overlap(c, f_in, f_out)) return BSL6D_EALIAS;
+    std::vector<Pass> passes;
+    int rc = plan_passes(c, sw, ns, passes);
+    if (rc) return rc;
+    if (passes.empty()) {
+        if (f_in != f_out) {
+            cudaError_t e = cudaMemcpyAsync(f_out, f_in, c->npts * sizeof(double), cudaMemcpyDeviceToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+        }
+        return BSL6D_OK;
+    }
+    const double* cur = f_in;
+    for (const Pass& p : passes) {
+        rc = launch_pass(c, cur, f_out, sw, p, st);
+        if (rc) return rc;
+        cur = f_out;
+    }
+    return BSL6D_OK;
+}
+
+// In place on f, ping-ponging with f_tmp when given; the result always lands in f.
+int run_sequence_pingpong(bsl6d_ctx* c, double* f, double* f_tmp, const SweepDesc* sw, int ns, cudaStream_t st) {
+    if (!c || !f) return BSL6D_EINVAL;
+    if (f_tmp && (f_tmp == f || partial_overlap(c, f, f_tmp))) return BSL6D_EALIAS;
+    std::vector<Pass> passes;
+    int rc = plan_passes(c, sw, ns, passes);
+    if (rc) return rc;
+    const int np = (int)passes.size();
+    double* cur = f;
+    double* other = f_tmp;
+    for (int s = 0; s < np; ++s) {
+        double* dst = cur;
+        if (other && !((np & 1) && s == 0)) dst = other;     // odd count: the first pass runs in place
+        rc = launch_pass(c, cur, dst, sw, passes[s], st);
+        if (rc) return rc;
+        if (dst != cur) { other = cur; cur = dst; }
+    }
     return BSL6D_OK;
 }
 
@@ -326,6 +510,7 @@ int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
     c->q = degree + 1;
     c->device = dev;
     c->npts = npts;
+    c->fusion = 1;
 
     std::vector<double> nodes(nn);
     size_t off = 0;
@@ -411,71 +596,71 @@ int bsl6d_rotate(bsl6d_ctx* c, const double* f_in, double* f_out, const double B
     int cnt = 0;
     int rc = plan_rotation(c, B, dt, sh, &cnt);
     if (rc) return rc;
-    const size_t bytes = c->npts * sizeof(double);
-    if (f_in != f_out) {
-        const char* a = (const char*)f_in;
-        const char* b = (const char*)f_out;
-        if (a < b + bytes && b < a + bytes) return BSL6D_EALIAS;
-    }
-    if (cnt == 0) {
-        if (f_in != f_out) {
-            cudaError_t e = cudaMemcpyAsync(f_out, f_in, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-        }
-        return BSL6D_OK;
-    }
-    const double* cur = f_in;
-    for (int i = 0; i < 3; ++i) {
-        rc = launch_sweep(c, cur, f_out, sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim,
-                          sh[i].scale, (cudaStream_t)stream);
-        if (rc) return rc;
-        cur = f_out;
-    }
-    return BSL6D_OK;
+    SweepDesc sw[3];
+    for (int i = 0; i < cnt; ++i)
+        sw[i] = SweepDesc{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
+    return run_sequence_in_out(c, f_in, f_out, sw, cnt, (cudaStream_t)stream);
 }
 
 int bsl6d_strang_step(bsl6d_ctx* c, double* f, double* f_tmp, const double* const E[3], const double B[3], double dt,
                       void* stream) {
     if (!c || !f || !std::isfinite(dt)) return BSL6D_EINVAL;
-    struct Step { int dim; const double* src; unsigned mask; double scale; };
-    Step steps[12];
+    SweepDesc steps[12];
     int ns = 0;
     const double half = 0.5 * dt;
     for (int d = 0; d < 3; ++d)
-        steps[ns++] = Step{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+        steps[ns++] = SweepDesc{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
     if (E)
         for (int d = 0; d < 3; ++d)
-            if (E[d]) steps[ns++] = Step{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
+            if (E[d]) steps[ns++] = SweepDesc{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
     if (B) {
         Shear sh[3];
         int cnt = 0;
         int rc = plan_rotation(c, B, dt, sh, &cnt);
         if (rc) return rc;
         for (int i = 0; i < cnt; ++i)
-            steps[ns++] = Step{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
+            steps[ns++] = SweepDesc{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
     }
     for (int d = 0; d < 3; ++d)
-        steps[ns++] = Step{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+        steps[ns++] = SweepDesc{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+    return run_sequence_pingpong(c, f, f_tmp, steps, ns, (cudaStream_t)stream);
+}
 
-    if (f_tmp) {
-        const size_t bytes = c->npts * sizeof(double);
-        const char* a = (const char*)f;
-        const char* b = (const char*)f_tmp;
-        if (a < b + bytes && b < a + bytes) return BSL6D_EALIAS;
+int bsl6d_advect_seq(bsl6d_ctx* c, const double* f_in, double* f_out, const bsl6d_sweep* sweeps, int nsweeps,
+                     void* stream) {
+    if (!c || nsweeps < 0 || nsweeps > 64 || (nsweeps > 0 && !sweeps)) return BSL6D_EINVAL;
+    SweepDesc sw[64];
+    for (int i = 0; i < nsweeps; ++i) {
+        const bsl6d_sweep& s = sweeps[i];
+        if (s.dim < 0 || s.dim > 5) return BSL6D_EINVAL;
+        if (!s.src && s.dim < 3)
+            sw[i] = SweepDesc{s.dim, c->d_nodes + c->node_off[s.dim + 3], 1u << (s.dim + 3), s.scale};
+        else
+            sw[i] = SweepDesc{s.dim, s.src, s.src_dim_mask, s.scale};
     }
-    // ping-pong f -> f_tmp -> f ...; with an odd number of sweeps the first one runs in place so that the
-    // result lands in f.  Without f_tmp everything runs in place.
-    double* cur = f;
-    double* other = f_tmp;
-    for (int s = 0; s < ns; ++s) {
-        double* dst = cur;
-        if (other && !((ns & 1) && s == 0)) dst = other;
-        int rc = launch_sweep(c, cur, dst, steps[s].dim, steps[s].src, steps[s].mask, steps[s].scale,
-                              (cudaStream_t)stream);
-        if (rc) return rc;
-        if (dst != cur) { other = cur; cur = dst; }
+    return run_sequence_in_out(c, f_in, f_out, sw, nsweeps, (cudaStream_t)stream);
+}
+
+int bsl6d_seq_passes(bsl6d_ctx* c, const bsl6d_sweep* sweeps, int nsweeps) {
+    if (!c || nsweeps < 0 || nsweeps > 64 || (nsweeps > 0 && !sweeps)) return BSL6D_EINVAL;
+    SweepDesc sw[64];
+    static const double dummy = 0.0;
+    for (int i = 0; i < nsweeps; ++i) {
+        const bsl6d_sweep& s = sweeps[i];
+        if (s.dim < 0 || s.dim > 5) return BSL6D_EINVAL;
+        if (!s.src && s.dim < 3) sw[i] = SweepDesc{s.dim, &dummy, 1u << (s.dim + 3), s.scale};
+        else sw[i] = SweepDesc{s.dim, s.src ? s.src : &dummy, s.src_dim_mask, s.scale};
     }
-    return BSL6D_OK;
+    std::vector<Pass> passes;
+    int rc = plan_passes(c, sw, nsweeps, passes);
+    return rc ? rc : (int)passes.size();
+}
+
+int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
+    if (!c) return BSL6D_EINVAL;
+    const int old = c->fusion;
+    c->fusion = enable ? 1 : 0;
+    return old;
 }
 
 int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {

@@ -23,21 +23,28 @@ namespace bsl6d {
 
 constexpr int kMaxSrcTerms = 5;
 
+// Where a pencil finds its shift source: the array seen along the swept dim is [outer][N][inner]; the source is a
+// dense C-order array over a subset of the other dims, so its index is a sum of up to five
+// (divide, modulo, stride) terms of the pencil's outer or inner index.
+struct SrcTerms {
+    uint32_t nterms;       // src index = sum_t ((g_t / below_t) % extent_t) * sstride_t,  g_t = outer or inner index
+    uint32_t t_inner[kMaxSrcTerms];   // 1: term decodes the inner index, 0: the outer index
+    uint32_t t_below[kMaxSrcTerms];
+    uint32_t t_extent[kMaxSrcTerms];  // 0 = slowest term of its group: no wrap needed
+    uint32_t t_sstride[kMaxSrcTerms];
+};
+
 struct SweepArgs {
     const double* in;
     double* out;
-    const double* src;     // shift source (device), indexed by the terms below
+    const double* src;     // shift source (device), indexed by `terms`
     double scale;          // alpha_cells = -(src * scale)
     uint32_t inner;        // product of extents of dims faster than the swept one
     uint32_t outer;        // product of extents of dims slower than the swept one
     uint32_t n;            // extent of the swept dim (== template N in the specialised kernels)
     uint32_t ti_log2;      // strided: threads of a block along `inner` = 1 << ti_log2
     uint32_t nib;          // strided: number of inner chunks (= ceil(inner / TI))
-    uint32_t nterms;       // src index = sum_t ((g_t / below_t) % extent_t) * sstride_t,  g_t = outer or inner index
-    uint32_t t_inner[kMaxSrcTerms];   // 1: term decodes the inner index, 0: the outer index
-    uint32_t t_below[kMaxSrcTerms];
-    uint32_t t_extent[kMaxSrcTerms];
-    uint32_t t_sstride[kMaxSrcTerms];
+    SrcTerms terms;
 };
 
 // ---- a2: Lagrange basis on the nodes m_i = i - Q/2 + 1, i = 0..Q-1 ------------------------------------------
@@ -88,12 +95,12 @@ __device__ __forceinline__ void split_shift(double a, double scale, long long& k
     k = (long long)kf;
 }
 
-__device__ __forceinline__ uint32_t src_offset(const SweepArgs& a, uint32_t o, uint32_t i) {
+__device__ __forceinline__ uint32_t src_offset(const SrcTerms& a, uint32_t o, uint32_t i) {
     uint32_t off = 0;
     for (uint32_t t = 0; t < a.nterms; ++t) {
         uint32_t g = a.t_inner[t] ? i : o;
         if (a.t_below[t] != 1u) g /= a.t_below[t];
-        if (a.t_extent[t] != 0u) g %= a.t_extent[t];      // extent 0 = "slowest term of its group": no wrap needed
+        if (a.t_extent[t] != 0u) g %= a.t_extent[t];
         off += g * a.t_sstride[t];
     }
     return off;
@@ -111,7 +118,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
 
     long long k;
     double theta;
-    split_shift(__ldg(a.src + src_offset(a, o, i)), a.scale, k, theta);
+    split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
 
     const size_t stride = a.inner;
     const size_t base = (size_t)o * N * stride + i;
@@ -182,7 +189,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_unit_kernel(const SweepArgs a) 
 
     // shift source first: its latency overlaps the tile load
     double sval = 0.0;
-    if (pl < np) sval = __ldg(a.src + src_offset(a, (uint32_t)(p0 + pl), 0u));
+    if (pl < np) sval = __ldg(a.src + src_offset(a.terms, (uint32_t)(p0 + pl), 0u));
 
 #pragma unroll
     for (int it = 0; it < (NE + T - 1) / T; ++it) {
@@ -247,7 +254,7 @@ __global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int
     const int n = (int)a.n;
     long long k;
     double theta;
-    split_shift(__ldg(a.src + src_offset(a, o, i)), a.scale, k, theta);
+    split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
     const size_t stride = a.inner;
     const size_t base = (size_t)o * n * stride + i;
     for (int r = 0; r < n; ++r) tile[r * T + threadIdx.x] = __ldcs(a.in + base + (size_t)r * stride);

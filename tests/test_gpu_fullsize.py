@@ -174,14 +174,14 @@ def test_C4_full_size_rotation_63_steps():
     b = torch.empty_like(a)
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
         for s in range(nsteps):
-            ctx.rotate(a, b, B, dt)                          # in -> out, then two shears in place (3 launches)
+            ctx.rotate(a, b, B, dt)                          # one fused pass in -> out (or 3 sweeps)
             a, b = b, a
             ref = oracle.rotate(ps.grid, w.degree, ref, B, dt)
             if s in (0, 1, 31, nsteps - 1):
                 got = ps.gather(a)
                 err = np.max(np.abs(got - ref)) / np.max(np.abs(ref))
                 assert err <= TOL, f"C4 step {s}: rel err {err:.3e}"
-        assert ctx.launch_count() == 3 * nsteps
+        assert ctx.launch_count() in (nsteps, 3 * nsteps)    # one fused pass per rotation where available
     # return to the initial state within interpolation error + smoothed noise: the GPU's global deviation is of
     # the size the oracle shows on the sampled planes (C4 is under-resolved in v2: ~3 % of max f)
     dev_oracle = np.max(np.abs(ref - ref0)) / np.max(np.abs(ref0))

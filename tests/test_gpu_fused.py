@@ -1,0 +1,180 @@
+"""Fused multi-sweep passes (include/bsl6d.h "sequences of sweeps"): a chain of sweeps run
+through the planner must give, bit for bit, what the same sweeps give one launch at a time, must agree with the
+oracle within 1e-12, and must take the number of passes the header promises."""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import bsl6d_workloads as wl
+import oracle
+import paper_2303_05994_b200 as bsl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+
+
+def ogrid(w):
+    return oracle.Grid(tuple(w.n), tuple(w.lo), tuple(w.dx))
+
+
+def six_sweeps(w, Ed):
+    """(dim, src, mask, scale) of x1,x2,x3 (grid nodes) then v1,v2,v3 (E_d over x)."""
+    sw = [(d, None, 0, w.dt / w.dx[d]) for d in range(3)]
+    sw += [(3 + d, Ed[d], 0x7, w.dt / w.dx[3 + d]) for d in range(3)]
+    return sw
+
+
+def rel_err(gpu: torch.Tensor, ref: np.ndarray) -> float:
+    return float(np.max(np.abs(gpu.cpu().numpy() - ref)) / np.max(np.abs(ref)))
+
+
+# grids whose extents all have fused kernels, for every stencil width; (n, degree, expected passes of the six sweeps)
+GRIDS = [
+    ((8, 8, 8, 8, 8, 8), 7, 4),           # (x1,x2) (x3,v1) v2 v3
+    ((8, 8, 8, 16, 16, 16), 5, 4),        # mixed (8,16) x3-v1 pair
+    ((16, 16, 16, 16, 16, 16), 9, 4),
+]
+
+
+@pytest.mark.parametrize("n,degree,npass", GRIDS)
+def test_six_sweeps_fused_equals_unfused_and_oracle(n, degree, npass):
+    _need_gpu()
+    w = wl.C2.reduced(n)
+    w = wl.replace(w, degree=degree)
+    f = w.make_f("cpu").numpy()
+    E = w.E()
+    Ed = [torch.from_numpy(e).cuda() for e in E]
+    fd = torch.from_numpy(f).cuda()
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        sw = six_sweeps(w, Ed)
+        assert ctx.seq_passes(sw) == npass
+        fused = ctx.advect_seq(fd, torch.empty_like(fd), sw)
+        l_fused = ctx.launch_count()
+        assert l_fused == npass
+        assert ctx.set_fusion(False) is True
+        assert ctx.seq_passes(sw) == 6
+        plain = ctx.advect_seq(fd, torch.empty_like(fd), sw)
+        assert ctx.launch_count() - l_fused == 6
+        inplace = fd.clone()
+        ctx.set_fusion(True)
+        ctx.advect_seq(inplace, inplace, sw)                 # fused passes in place
+    assert torch.equal(fused, plain)
+    assert torch.equal(fused, inplace)
+    ref = f
+    for d in range(6):
+        ref = oracle.advect(ogrid(w), w.degree, ref, d, None if d < 3 else E[d - 3], w.dt)
+    assert rel_err(fused, ref) <= TOL
+
+
+@pytest.mark.parametrize("n,degree", [((2, 3, 2, 8, 8, 8), 7), ((2, 2, 2, 16, 16, 16), 5), ((1, 2, 1, 32, 32, 32), 7),
+                                      ((1, 1, 2, 48, 48, 8), 9), ((1, 1, 1, 64, 64, 16), 5)])
+def test_rotation_fused_equals_unfused_and_oracle(n, degree):
+    """B along x3: the three shears v1, v2, v1 are one ABA pass; |alpha| reaches 1.6 cells (k != 0)."""
+    _need_gpu()
+    w = wl.C4.reduced(n)
+    w = wl.replace(w, degree=degree)
+    f = w.make_f("cpu").numpy()
+    fd = torch.from_numpy(f).cuda()
+    B, dt = (0.0, 0.0, 1.0), 0.1
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        fused = ctx.rotate(fd, torch.empty_like(fd), B, dt)
+        assert ctx.launch_count() == 1
+        ctx.set_fusion(False)
+        plain = ctx.rotate(fd, torch.empty_like(fd), B, dt)
+        assert ctx.launch_count() == 4
+        ctx.set_fusion(True)
+        inplace = fd.clone()
+        ctx.rotate(inplace, inplace, B, -dt)                 # negative angle, in place
+        ctx.set_fusion(False)
+        plain_neg = ctx.rotate(fd, torch.empty_like(fd), B, -dt)
+    assert torch.equal(fused, plain)
+    assert torch.equal(inplace, plain_neg)
+    assert rel_err(fused, oracle.rotate(ogrid(w), w.degree, f, B, dt)) <= TOL
+
+
+def test_rotation_other_axes_fall_back_to_single_sweeps():
+    """B along x1 / x2 involves the unit-stride dim v3: no fused kernel, three launches, same numbers as before."""
+    _need_gpu()
+    w = wl.C4.reduced((2, 2, 2, 16, 16, 16))
+    f = w.make_f("cpu").numpy()
+    fd = torch.from_numpy(f).cuda()
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for ax in (0, 1):
+            B = [0.0, 0.0, 0.0]
+            B[ax] = 1.0
+            before = ctx.launch_count()
+            out = ctx.rotate(fd, torch.empty_like(fd), B, 0.1)
+            assert ctx.launch_count() - before == 3
+            assert rel_err(out, oracle.rotate(ogrid(w), w.degree, f, B, 0.1)) <= TOL
+
+
+@pytest.mark.parametrize("pingpong", (False, True))
+def test_strang_step_fused_equals_unfused_and_oracle(pingpong):
+    _need_gpu()
+    w = wl.C5.reduced((8, 8, 8, 16, 16, 16))
+    f = w.make_f("cpu").numpy()
+    E = w.E()
+    Ed = [torch.from_numpy(e).cuda() for e in E]
+    a = torch.from_numpy(f).cuda()
+    b = a.clone()
+    tmp = torch.empty_like(a) if pingpong else None
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for _ in range(2):
+            ctx.strang_step(a, tmp, Ed, w.B, w.dt)
+        # (x1,x2) (x3,v1) v2 v3 (v1,v2,v1) (x1,x2) x3 = 7 passes per step
+        assert ctx.launch_count() == 14
+        ctx.set_fusion(False)
+        for _ in range(2):
+            ctx.strang_step(b, tmp, Ed, w.B, w.dt)
+        assert ctx.launch_count() == 14 + 24
+    assert torch.equal(a, b)
+    ref = f.copy()
+    for _ in range(2):
+        ref = oracle.strang_step(ogrid(w), w.degree, ref, E, w.B, w.dt)
+    assert rel_err(a, ref) <= TOL
+
+
+def test_integer_shifts_stay_bit_exact_through_fused_passes():
+    """Whole-cell displacements in both sweeps of a fused pair: the pass is an exact permutation (x, periodic)
+    followed by an exact shift with zero fill (v)."""
+    _need_gpu()
+    w = wl.C2.reduced((8, 8, 8, 8, 8, 8))
+    f = w.make_f("cpu").numpy()
+    fd = torch.from_numpy(f).cuda()
+    one = torch.ones(1, dtype=torch.float64, device="cuda")
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        sw = [(0, one, 0, 3.0), (1, one, 0, -2.0), (2, one, 0, 1.0), (3, one, 0, 2.0)]   # alpha = -3, +2, -1, -2 cells
+        assert ctx.seq_passes(sw) == 2
+        out = ctx.advect_seq(fd, torch.empty_like(fd), sw).cpu().numpy()
+    ref = np.roll(np.roll(np.roll(f, 3, axis=0), -2, axis=1), 1, axis=2)
+    exp = np.zeros_like(ref)
+    exp[:, :, :, 2:] = ref[:, :, :, :-2]                     # out[j] = in[j-2], zero fill
+    assert np.array_equal(out, exp)
+
+
+def test_sequence_error_paths_enqueue_nothing():
+    _need_gpu()
+    w = wl.C1
+    fd = w.make_f("cuda")
+    one = torch.ones(1, dtype=torch.float64, device="cuda")
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_seq(fd, fd, [(0, None, 0, 0.1), (3, None, 0x7, 0.1)])   # v sweep without a source
+        assert e.value.code == bsl.EINVAL
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_seq(fd, fd, [(0, None, 0, 0.1), (1, one, 1 << 1, 0.1)])  # mask contains the swept dim
+        assert e.value.code == bsl.EINVAL
+        with pytest.raises(bsl.Bsl6dError):
+            ctx.advect_seq(fd, fd, [(0, None, 0, float("inf"))])
+        assert ctx.launch_count() == 0
+        out = ctx.advect_seq(fd, torch.empty_like(fd), [])   # empty chain copies
+        assert torch.equal(out, fd)

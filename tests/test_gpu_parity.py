@@ -250,7 +250,7 @@ def test_C4_reduced_rotation_return_63_steps():
             ctx.rotate(cur, cur, w.B, theta)
             ref = oracle.rotate(ogrid(w), w.degree, ref, w.B, theta)
         rel = assert_close(cur, ref, "C4r 63 rotations")
-        assert ctx.launch_count() == 189
+        assert ctx.launch_count() in (63, 189)                # one fused pass per rotation, or three sweeps
     back = np.max(np.abs(ref - f0)) / np.max(np.abs(f0))
     assert back < 0.06, back                                  # under-resolved on purpose (sigma_v2 = 0.5, dv = 0.375)
     print(f"C4r: gpu-vs-oracle {rel:.2e}, return error {back:.3e}")
@@ -273,14 +273,14 @@ def test_C5_reduced_strang_steps_and_density(pingpong):
             assert_close(cur, ref, f"C5r step {step}")
             ctx.density(cur, rho)
             assert_close(rho, oracle.density(ogrid(w), ref), f"C5r rho step {step}")
-        assert ctx.launch_count() == 3 * 13
+        assert ctx.launch_count() in (3 * 10, 3 * 13)         # fused v1v2 + fused shears, or 12 sweeps; + density
         # no E, no B: 6 sweeps; E only: 9 sweeps (odd count with ping-pong still lands in f)
         before = ctx.launch_count()
         ctx.strang_step(cur, tmp, None, None, w.dt)
         ref = oracle.strang_step(ogrid(w), w.degree, ref, [None] * 3, None, w.dt)
         ctx.strang_step(cur, tmp, Ed, None, w.dt)
         ref = oracle.strang_step(ogrid(w), w.degree, ref, E, None, w.dt)
-        assert ctx.launch_count() - before == 15
+        assert ctx.launch_count() - before in (14, 15)
         assert_close(cur, ref, "C5r partial steps")
 
 
