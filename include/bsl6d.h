@@ -105,8 +105,10 @@ BSL6D_API int bsl6d_strang_step(bsl6d_ctx* ctx, double* f, double* f_tmp, const 
  * arithmetic is unchanged, so the numbers are bit-identical to issuing the sweeps one by one.
  * bsl6d_rotate, bsl6d_strang_step and bsl6d_advect_seq all go through this planner; a group without a fused
  * kernel (extent not in {8,16,32,48,64}, degree not in {5,7,9}, inner extent not a multiple of C) silently runs
- * as single sweeps.  bsl6d_set_fusion(ctx, 0) turns grouping off (every sweep its own pass); returns the old
- * setting (default 1). */
+ * as single sweeps, and so does a PAIR that measurement says does not pay (row segments under 64 bytes, or a tile
+ * whose rows lie >= 64 MB apart).  The planner picks the grouping with the fewest passes.
+ * bsl6d_set_fusion(ctx, 0) turns grouping off (every sweep its own pass), 1 is the default policy, 2 fuses
+ * wherever a kernel exists (for tests and tuning); returns the old setting. */
 typedef struct bsl6d_sweep {
     int32_t dim;             /* swept dim 0..5 */
     uint32_t src_dim_mask;   /* dims the shift source is dense over (bit d), must not contain `dim` */

@@ -209,11 +209,12 @@ class Context:
             self._check(rc, "bsl6d_seq_passes")
         return rc
 
-    def set_fusion(self, enable: bool) -> bool:
-        rc = self._lib.bsl6d_set_fusion(self._h, 1 if enable else 0)
+    def set_fusion(self, mode) -> int:
+        """0 / False: off; 1 / True: default policy; 2: fuse wherever a kernel exists.  Returns the old mode."""
+        rc = self._lib.bsl6d_set_fusion(self._h, int(mode))
         if rc < 0:
             self._check(rc, "bsl6d_set_fusion")
-        return bool(rc)
+        return rc
 
     def density(self, f, rho, stream=None):
         self._shape_ok(f, "f")

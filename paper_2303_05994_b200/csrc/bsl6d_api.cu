@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -27,8 +28,9 @@ struct bsl6d_ctx {
     size_t dens_chunk;
     int last_cuda;
     long long launches;
+    int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
-    const void* smem_ok[16];  // fused kernels whose dynamic shared-memory limit has been raised
+    const void* smem_ok[32];  // fused kernels whose dynamic shared-memory limit has been raised
     int n_smem_ok;
     // host-path working set (bsl6d_run_host), allocated on first use
     double* h_f;              // device buffer for f
@@ -320,6 +322,12 @@ bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) 
     if (!fused_lookup(c->q, n[a], n[b], a < 3, b < 3, pattern, fc)) return false;
     if (inner_b % (size_t)fc.C) return false;
     if (c->npts > 0xFFFFFFFFull) return false;                        // 32-bit pencil indices in the kernel
+    // Policy from measurement: a pair only pays with >= 64-byte row segments and a tile whose
+    // rows are not spread over hundreds of MB (x1 on the big grids); the three-sweep rotation always pays.
+    if (cnt == 2 && !c->fuse_all) {
+        const size_t strideA_bytes = mid * (size_t)n[b] * inner_b * sizeof(double);
+        if (fc.C < 8 || strideA_bytes >= ((size_t)64 << 20)) return false;
+    }
     const size_t blocks = outer * mid * (inner_b / (size_t)fc.C);
     if (blocks > 0x7FFFFFFFull) return false;
     p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern;
@@ -335,15 +343,26 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
         rc = choose_kernel(c, sw[i].dim, kc);
         if (rc) return rc;
     }
-    int i = 0;
-    while (i < ns) {
-        Pass p{i, 1, false, {}, 0};
-        if (c->fusion) {
-            if (!(i + 2 < ns && try_fuse(c, sw, i, 3, p)))
-                if (i + 1 < ns) (void)try_fuse(c, sw, i, 2, p);
+    // Fewest passes over the chain (dynamic programme from the back): a group of 3 (a,b,a), 2 (a,b) or 1 sweeps.
+    std::vector<int> best(ns + 1, 0), pick(ns + 1, 1);
+    std::vector<Pass> cand2(ns), cand3(ns);
+    std::vector<char> ok2(ns, 0), ok3(ns, 0);
+    for (int i = ns - 1; i >= 0; --i) {
+        best[i] = 1 + best[i + 1];
+        pick[i] = 1;
+        if (c->fusion && i + 1 < ns && try_fuse(c, sw, i, 2, cand2[i])) {
+            ok2[i] = 1;
+            if (1 + best[i + 2] < best[i]) { best[i] = 1 + best[i + 2]; pick[i] = 2; }
         }
-        passes.push_back(p);
-        i += p.count;
+        if (c->fusion && i + 2 < ns && try_fuse(c, sw, i, 3, cand3[i])) {
+            ok3[i] = 1;
+            if (1 + best[i + 3] < best[i]) { best[i] = 1 + best[i + 3]; pick[i] = 3; }
+        }
+    }
+    for (int i = 0; i < ns; i += pick[i]) {
+        if (pick[i] == 3) passes.push_back(cand3[i]);
+        else if (pick[i] == 2) passes.push_back(cand2[i]);
+        else passes.push_back(Pass{i, 1, false, {}, 0});
     }
     return BSL6D_OK;
 }
@@ -377,7 +396,7 @@ int launch_fused(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDes
         if (!known) {
             e = cudaFuncSetAttribute(p.fc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.fc.smem);
             if (e != cudaSuccess) return cuda_fail(c, e);
-            if (c->n_smem_ok < 16) c->smem_ok[c->n_smem_ok++] = p.fc.fn;
+            if (c->n_smem_ok < 32) c->smem_ok[c->n_smem_ok++] = p.fc.fn;
         }
     }
     const unsigned grid = (unsigned)(outer * mid * (size_t)fa.nchunks);
@@ -511,6 +530,7 @@ int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
     c->device = dev;
     c->npts = npts;
     c->fusion = 1;
+    c->fuse_all = 0;
 
     std::vector<double> nodes(nn);
     size_t off = 0;
@@ -658,8 +678,9 @@ int bsl6d_seq_passes(bsl6d_ctx* c, const bsl6d_sweep* sweeps, int nsweeps) {
 
 int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     if (!c) return BSL6D_EINVAL;
-    const int old = c->fusion;
+    const int old = c->fusion ? (c->fuse_all ? 2 : 1) : 0;
     c->fusion = enable ? 1 : 0;
+    c->fuse_all = enable == 2 ? 1 : 0;
     return old;
 }
 

@@ -8,7 +8,7 @@
 //
 //   phase "a, global -> smem":  thread (ib, c) loads its column along a from global memory in shifted order into
 //                               registers (exactly the strided sweep kernel), sweeps, writes the column into the tile
-//   phase "b, smem -> smem":    thread (ia, c) reads its row along b from the tile, sweeps, barrier, writes it back
+//   phase "b, smem -> smem":    thread (ia, c) reads its row along b from the tile, sweeps, writes it back in place
 //   phase "b, smem -> global":  the same, results streamed to global memory (segments of C contiguous doubles)
 //   phase "a, smem -> global":  thread (ib, c) reads its column from the tile, sweeps, streams it out
 //
@@ -147,27 +147,20 @@ __global__ void __launch_bounds__(FusedGeom<NA, NB, C>::T, MINB) sweep_fused_ker
         return;
     }
 
-    // PATTERN == kPatABA: b in place in the tile, then a from the tile to global memory
-    {
-        double res[G::RB][NB];
+    // PATTERN == kPatABA: b in place in the tile (a thread owns its whole row: it has read all of it into registers
+    // before it writes any of it back), then a from the tile to global memory
 #pragma unroll
-        for (int r = 0; r < G::RB; ++r) {
-            const uint32_t p = r * T + threadIdx.x;
-            const uint32_t ia = p / C, c = p % C;
-            const uint32_t outer_idx = (o * NA + ia) * a.mid + m;
-            const double sval = __ldg(a.sw[1].src + src_offset(a.sw[1].terms, outer_idx, i0 + c));
-            sweep_pencil<NB, Q, PB, false>(tile + ia * LDS + c, (size_t)C, sval, a.sw[1].scale, res[r]);
-        }
-        __syncthreads();                                   // every row has been read
+    for (int r = 0; r < G::RB; ++r) {
+        const uint32_t p = r * T + threadIdx.x;
+        const uint32_t ia = p / C, c = p % C;
+        const uint32_t outer_idx = (o * NA + ia) * a.mid + m;
+        const double sval = __ldg(a.sw[1].src + src_offset(a.sw[1].terms, outer_idx, i0 + c));
+        double res[NB];
+        sweep_pencil<NB, Q, PB, false>(tile + ia * LDS + c, (size_t)C, sval, a.sw[1].scale, res);
 #pragma unroll
-        for (int r = 0; r < G::RB; ++r) {
-            const uint32_t p = r * T + threadIdx.x;
-            const uint32_t ia = p / C, c = p % C;
-#pragma unroll
-            for (int j = 0; j < NB; ++j) tile[ia * LDS + j * C + c] = res[r][j];
-        }
-        __syncthreads();
+        for (int j = 0; j < NB; ++j) tile[ia * LDS + j * C + c] = res[j];
     }
+    __syncthreads();
 #pragma unroll
     for (int r = 0; r < G::RA; ++r) {
         const uint32_t p = r * T + threadIdx.x;

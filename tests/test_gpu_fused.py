@@ -60,7 +60,7 @@ def test_six_sweeps_fused_equals_unfused_and_oracle(n, degree, npass):
         fused = ctx.advect_seq(fd, torch.empty_like(fd), sw)
         l_fused = ctx.launch_count()
         assert l_fused == npass
-        assert ctx.set_fusion(False) is True
+        assert ctx.set_fusion(False) == 1
         assert ctx.seq_passes(sw) == 6
         plain = ctx.advect_seq(fd, torch.empty_like(fd), sw)
         assert ctx.launch_count() - l_fused == 6
