@@ -157,3 +157,16 @@ def strang_step(grid: Grid, degree: int, f: np.ndarray, E: Sequence[Optional[np.
     _check(_load().oracle_strang_step(n, lo, dx, degree, _dp(f), _dp(Es[0]), _dp(Es[1]), _dp(Es[2]), Bc, float(dt)),
            "strang_step")
     return f
+
+
+# ---- field step: plain numpy, see oracle/fields.py ------------------------------------------
+from . import fields as _fields  # noqa: E402
+import sys as _sys  # noqa: E402
+
+poisson_E = _fields.poisson_E
+adiabatic_E = _fields.adiabatic_E
+
+
+def vp_step(grid, degree, f, B, dt, closure="poisson", c1=1.0, e_fac=1.0):
+    """Self-consistent Strang step (oracle/fields.py::vp_step) using this module's sweeps and density."""
+    return _fields.vp_step(_sys.modules[__name__], grid, degree, f, B, dt, closure, c1, e_fac)
