@@ -127,6 +127,27 @@ BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);
 
+/* ---- field step: the self-consistent electric field ------------------------------------------
+ * PAPER.md:44-48 eq (2): rho_c = q (int f dv - n0), -Laplace(phi) = rho_c, E = -grad(phi), solved pseudo-spectrally on
+ * the periodic x grid; eq (11): the adiabatic-electron closure (n0 q^2/T_e) phi = rho_c.
+ * rho is the bare moment of bsl6d_density (n0*n1*n2 doubles, DEVICE).  The neutralising background n0 is the mean of
+ * the moment (the k = 0 mode is dropped, reading F1); Nyquist modes have no first derivative (reading F2).
+ *   poisson:    E_d <- e_fac * ( -d/dx_d phi ),   -Laplace(phi) = rho_fac * (rho - mean)
+ *   adiabatic:  E_d <- e_fac * ( -d/dx_d phi ),    phi = phi_fac * (rho - mean)
+ * E: HOST array of three DEVICE pointers (outputs, n0*n1*n2 doubles each).  With e_fac = q/m the outputs are exactly
+ * the shift sources bsl6d_advect wants for dims 3..5.  The transform is a hand-written separable DFT (any extent);
+ * 13 small launches on the caller's stream. */
+BSL6D_API int bsl6d_field_poisson(bsl6d_ctx* ctx, const double* rho, double rho_fac, double e_fac, double* const E[3],
+                        void* stream);
+BSL6D_API int bsl6d_field_adiabatic(bsl6d_ctx* ctx, const double* rho, double phi_fac, double e_fac, double* const E[3],
+                          void* stream);
+/* One self-consistent Strang step (Fig. 1 caption at 114), result in f:
+ *   x1,x2,x3 (dt/2) -> rho = moment(f) -> field solve -> v1,v2,v3 with E (dt) -> rotation (B may be NULL) -> x1,x2,x3 (dt/2).
+ * closure 0 = Poisson (c1 = rho_fac), 1 = adiabatic (c1 = phi_fac).  rho and E[0..2] are caller-owned DEVICE work
+ * buffers and hold the mid-step moment and field on return.  f_tmp as in bsl6d_strang_step. */
+BSL6D_API int bsl6d_vp_step(bsl6d_ctx* ctx, double* f, double* f_tmp, double* rho, double* const E[3], const double B[3],
+                  double dt, int closure, double c1, double e_fac, void* stream);
+
 /* ---- end-to-end entry point on HOST buffers -------------------------------------------------------------
  * Runs a sequence of operations on a distribution function that lives in HOST memory (pinned for full speed):
  * copies f_in_host to the device, runs the ops back to back on an internal stream, copies the result to

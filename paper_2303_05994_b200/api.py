@@ -19,7 +19,7 @@ SYMBOLS = (
     "bsl6d_create", "bsl6d_destroy", "bsl6d_advect", "bsl6d_advect_generic", "bsl6d_rotate",
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
-    "bsl6d_set_fusion",
+    "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
 )
 
 OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
@@ -79,6 +79,10 @@ def load_library() -> C.CDLL:
     lib.bsl6d_advect_seq.argtypes = [vp, dp, dp, C.POINTER(Sweep), C.c_int, vp]
     lib.bsl6d_seq_passes.argtypes = [vp, C.POINTER(Sweep), C.c_int]
     lib.bsl6d_set_fusion.argtypes = [vp, C.c_int]
+    lib.bsl6d_field_poisson.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
+    lib.bsl6d_field_adiabatic.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
+    lib.bsl6d_vp_step.argtypes = [vp, dp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, C.c_int,
+                                  C.c_double, C.c_double, vp]
     _lib = lib
     return lib
 
@@ -215,6 +219,31 @@ class Context:
         if rc < 0:
             self._check(rc, "bsl6d_set_fusion")
         return rc
+
+    def _E3(self, E):
+        nx = self.n[0] * self.n[1] * self.n[2]
+        for e in E:
+            if e.numel() != nx:
+                raise ValueError("E: wrong number of elements")
+        return (C.c_void_p * 3)(*[_dev_ptr(e, "E") for e in E])
+
+    def field_poisson(self, rho, rho_fac: float, e_fac: float, E, stream=None):
+        self._check(self._lib.bsl6d_field_poisson(self._h, _dev_ptr(rho, "rho"), float(rho_fac), float(e_fac),
+                                                  self._E3(E), _stream(stream)), "bsl6d_field_poisson")
+        return E
+
+    def field_adiabatic(self, rho, phi_fac: float, e_fac: float, E, stream=None):
+        self._check(self._lib.bsl6d_field_adiabatic(self._h, _dev_ptr(rho, "rho"), float(phi_fac), float(e_fac),
+                                                    self._E3(E), _stream(stream)), "bsl6d_field_adiabatic")
+        return E
+
+    def vp_step(self, f, f_tmp, rho, E, B, dt: float, closure: int, c1: float, e_fac: float, stream=None):
+        self._shape_ok(f, "f")
+        Bc = None if B is None else (C.c_double * 3)(*[float(b) for b in B])
+        self._check(self._lib.bsl6d_vp_step(self._h, _dev_ptr(f, "f"), _dev_ptr(f_tmp, "f_tmp"), _dev_ptr(rho, "rho"),
+                                            self._E3(E), Bc, float(dt), int(closure), float(c1), float(e_fac),
+                                            _stream(stream)), "bsl6d_vp_step")
+        return f
 
     def density(self, f, rho, stream=None):
         self._shape_ok(f, "f")

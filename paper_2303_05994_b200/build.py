@@ -26,7 +26,7 @@ UNITS = [
     ("bsl6d_fused_q8.o", "bsl6d_fused.cu", ["-DBSL6D_FUSED_Q=8"]),
     ("bsl6d_fused_q10.o", "bsl6d_fused.cu", ["-DBSL6D_FUSED_Q=10"]),
 ]
-HEADERS = ["sweep_kernels.cuh", "density_kernels.cuh", "fused_kernels.cuh", "fused_api.h",
+HEADERS = ["sweep_kernels.cuh", "density_kernels.cuh", "fused_kernels.cuh", "fused_api.h", "field_kernels.cuh",
            os.path.join("..", "..", "include", "bsl6d.h")]
 
 NVCC_FLAGS = [

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "density_kernels.cuh"
+#include "field_kernels.cuh"
 #include "fused_api.h"
 #include "fused_kernels.cuh"
 #include "sweep_kernels.cuh"
@@ -28,6 +29,8 @@ struct bsl6d_ctx {
     size_t dens_chunk;
     int last_cuda;
     long long launches;
+    double2* fld[5];          // field step: complex work arrays over the x grid (allocated on first use)
+    double2* tw[3];           // field step: twiddle tables exp(-2 pi i m / n_d)
     int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
     const void* smem_ok[32];  // fused kernels whose dynamic shared-memory limit has been raised
@@ -489,6 +492,59 @@ int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear out[3]
     return BSL6D_OK;
 }
 
+// ---- field step ------------------------------------------------------------------------------
+int field_setup(bsl6d_ctx* c) {
+    if (c->fld[0]) return BSL6D_OK;
+    const size_t nx = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2];
+    if (nx > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+    for (int d = 0; d < 3; ++d) {
+        const int n = c->g.n[d];
+        std::vector<double2> w((size_t)n);
+        for (int m = 0; m < n; ++m) {
+            const double ang = -2.0 * 3.14159265358979323846 * (double)m / (double)n;
+            w[(size_t)m] = make_double2(std::cos(ang), std::sin(ang));
+        }
+        if (cudaMalloc((void**)&c->tw[d], (size_t)n * sizeof(double2)) != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+        cudaError_t e = cudaMemcpy(c->tw[d], w.data(), (size_t)n * sizeof(double2), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+    for (int k = 4; k >= 0; --k)                               // fld[0] last: it marks "set up"
+        if (cudaMalloc((void**)&c->fld[k], nx * sizeof(double2)) != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+    return BSL6D_OK;
+}
+
+int field_solve(bsl6d_ctx* c, const double* rho, int adiabatic, double c1, double e_fac, double* const E[3],
+                cudaStream_t st) {
+    if (!c || !rho || !E || !E[0] || !E[1] || !E[2]) return BSL6D_EINVAL;
+    if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
+    int rc = field_setup(c);
+    if (rc) return rc;
+    const uint32_t n0 = (uint32_t)c->g.n[0], n1 = (uint32_t)c->g.n[1], n2 = (uint32_t)c->g.n[2];
+    const uint32_t total = n0 * n1 * n2;
+    const unsigned T = 128, grid = (total + T - 1) / T;
+    double2 *A = c->fld[0], *B = c->fld[1];
+    using namespace bsl6d;
+    // forward: axis 2 (real in), axis 1, axis 0
+    dft_axis_kernel<true, false><<<grid, T, 0, st>>>(rho, A, c->tw[2], n2, 1u, total, 0, 1.0);
+    dft_axis_kernel<false, false><<<grid, T, 0, st>>>(A, B, c->tw[1], n1, n2, total, 0, 1.0);
+    dft_axis_kernel<false, false><<<grid, T, 0, st>>>(B, A, c->tw[0], n0, n1 * n2, total, 0, 1.0);
+    FieldArgs fa;
+    for (int d = 0; d < 3; ++d) { fa.n[d] = (uint32_t)c->g.n[d]; fa.L[d] = (double)c->g.n[d] * c->g.dx[d]; }
+    fa.adiabatic = adiabatic;
+    fa.c1 = c1;
+    spectral_field_kernel<<<grid, T, 0, st>>>(A, c->fld[2], c->fld[3], c->fld[4], fa);
+    const double scale = e_fac / (double)total;
+    for (int d = 0; d < 3; ++d) {
+        dft_axis_kernel<false, false><<<grid, T, 0, st>>>(c->fld[2 + d], A, c->tw[0], n0, n1 * n2, total, 1, 1.0);
+        dft_axis_kernel<false, false><<<grid, T, 0, st>>>(A, B, c->tw[1], n1, n2, total, 1, 1.0);
+        dft_axis_kernel<false, true><<<grid, T, 0, st>>>(B, E[d], c->tw[2], n2, 1u, total, 1, scale);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 13;
+    return BSL6D_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -570,6 +626,8 @@ void bsl6d_destroy(bsl6d_ctx* c) {
     if (c->h_stream) { cudaStreamSynchronize(c->h_stream); cudaStreamDestroy(c->h_stream); }
     cudaFree(c->h_f);
     cudaFree(c->h_small);
+    for (int k = 0; k < 5; ++k) cudaFree(c->fld[k]);
+    for (int k = 0; k < 3; ++k) cudaFree(c->tw[k]);
     cudaFree(c->d_part);
     cudaFree(c->d_nodes);
     (void)cudaGetLastError();
@@ -682,6 +740,47 @@ int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     c->fusion = enable ? 1 : 0;
     c->fuse_all = enable == 2 ? 1 : 0;
     return old;
+}
+
+int bsl6d_field_poisson(bsl6d_ctx* c, const double* rho, double rho_fac, double e_fac, double* const E[3],
+                        void* stream) {
+    return field_solve(c, rho, 0, rho_fac, e_fac, E, (cudaStream_t)stream);
+}
+
+int bsl6d_field_adiabatic(bsl6d_ctx* c, const double* rho, double phi_fac, double e_fac, double* const E[3],
+                          void* stream) {
+    return field_solve(c, rho, 1, phi_fac, e_fac, E, (cudaStream_t)stream);
+}
+
+int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* const E[3], const double B[3],
+                  double dt, int closure, double c1, double e_fac, void* stream) {
+    if (!c || !f || !rho || !E || !E[0] || !E[1] || !E[2] || !std::isfinite(dt)) return BSL6D_EINVAL;
+    if (closure != 0 && closure != 1) return BSL6D_EINVAL;
+    if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
+    Shear sh[3];
+    int cnt = 0;
+    if (B) {
+        int rc = plan_rotation(c, B, dt, sh, &cnt);
+        if (rc) return rc;
+    }
+    int rc = field_setup(c);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const double half = 0.5 * dt;
+    SweepDesc xs[3], vs[9];
+    for (int d = 0; d < 3; ++d) xs[d] = SweepDesc{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
+    int nv = 0;
+    for (int d = 0; d < 3; ++d) vs[nv++] = SweepDesc{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
+    for (int i = 0; i < cnt; ++i)
+        vs[nv++] = SweepDesc{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
+    for (int d = 0; d < 3; ++d) vs[nv++] = xs[d];
+    rc = run_sequence_pingpong(c, f, f_tmp, xs, 3, st);
+    if (rc) return rc;
+    rc = bsl6d_density(c, f, rho, stream);
+    if (rc) return rc;
+    rc = field_solve(c, rho, closure, c1, e_fac, E, st);
+    if (rc) return rc;
+    return run_sequence_pingpong(c, f, f_tmp, vs, nv, st);
 }
 
 int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
