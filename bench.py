@@ -380,6 +380,28 @@ def run_ours(args, w):
                  "note": "same nine sweeps + density, bit-identical results; consecutive sweeps over two dims share one "
                          "pass over f (bsl6d_advect_seq: x1 | x2+x3 | v1+v2 | v3; bsl6d_rotate: one pass), so bytes per "
                          "point-update drop below 16 and the per-sweep roofline does not apply"}
+        # the full Strang step of BASELINE configs[4] on this grid (12 sweeps; x half, E, rotation, x half)
+        def time_strang(mode):
+            ctx.set_fusion(mode)
+            l0_ = ctx.launch_count()
+            for _ in range(2):
+                ctx.strang_step(cur, oth, E, ROT_B, w.dt)
+            barrier()
+            per = (ctx.launch_count() - l0_) // 2
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record(stream)
+            for _ in range(K):
+                ctx.strang_step(cur, oth, E, ROT_B, w.dt)
+            s1.record(stream)
+            barrier()
+            return max_over_ranks(s0.elapsed_time(s1), dev) / K, per
+
+        st_f, lp_f = time_strang(1)
+        st_u, lp_u = time_strang(0)
+        fused["strang_step"] = {"ms_fused": st_f, "launches_fused": lp_f, "ms_per_sweep_path": st_u,
+                                "launches_per_sweep_path": lp_u,
+                                "Gpoint-updates/s_fused": 12 * npts / (st_f * 1e-3) / 1e9,
+                                "Gpoint-updates/s_per_sweep_path": 12 * npts / (st_u * 1e-3) / 1e9}
         ctx.set_fusion(0)
 
     # ---- e2e: the same step through bsl6d_run_host on HOST buffers (pinned), copies inside the timed region
