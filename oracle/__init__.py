@@ -47,6 +47,8 @@ def _load():
         lib.oracle_rotate.argtypes = [ip, dp, dp, C.c_int, dp, dp, dp, C.c_double]
         lib.oracle_density.argtypes = [ip, dp, dp, dp]
         lib.oracle_strang_step.argtypes = [ip, dp, dp, C.c_int, dp, dp, dp, dp, dp, C.c_double]
+        lib.oracle_lagrange_weights_odd.argtypes = [C.c_int, C.c_double, dp]
+        lib.oracle_sweep_pointwise.argtypes = [ip, dp, dp, C.c_int, dp, C.c_int]
         _lib = lib
     return _lib
 
@@ -114,6 +116,25 @@ def sweep(f_in: np.ndarray, dim: int, src: np.ndarray, src_mask: int, scale: flo
     if out is None:
         out = np.empty_like(f_in)
     _check(_load().oracle_sweep(n, _dp(f_in), _dp(out), dim, _dp(src), src_mask, float(scale), q), "sweep")
+    return out
+
+
+def lagrange_weights_odd(q: int, alpha: float) -> np.ndarray:
+    """l_m(alpha) on the nodes m = -(q-1)/2 .. (q-1)/2, odd q  (eq (6))."""
+    w = np.empty(q, dtype=np.float64)
+    _check(_load().oracle_lagrange_weights_odd(q, float(alpha), _dp(w)), "lagrange_weights_odd")
+    return w
+
+
+def sweep_pointwise(f_in: np.ndarray, dim: int, alpha_cells: np.ndarray, q: int,
+                    out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Odd-q sweep along `dim` with one displacement per point (alpha_cells has f's shape), eq (6)."""
+    assert f_in.ndim == 6 and alpha_cells.shape == f_in.shape
+    n = (C.c_int32 * 6)(*f_in.shape)
+    alpha_cells = np.ascontiguousarray(alpha_cells, dtype=np.float64)
+    if out is None:
+        out = np.empty_like(f_in)
+    _check(_load().oracle_sweep_pointwise(n, _dp(f_in), _dp(out), dim, _dp(alpha_cells), q), "sweep_pointwise")
     return out
 
 

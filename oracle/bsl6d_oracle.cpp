@@ -25,6 +25,8 @@
 //   rotate             pinned (2x2 shear product = rotation matrix, closed-form rotated Gaussian, 2*pi return)
 //   density            pinned (math.fsum brute force, Maxwellian closed form)
 //   strang_step        pinned compositionally + E=0,B=0 free-streaming closed form + E-only closed form
+//   sweep_pointwise    pinned (odd-q weights: closed forms and exact rationals; polynomial reproduction with
+//                      per-point alpha; whole-cell alpha = exact roll; numpy polynomial interpolation per point)
 //
 #include <cmath>
 #include <cstdint>
@@ -81,6 +83,44 @@ void pencil_update(int n, int q, bool periodic, const double* g, double a, doubl
             } else {
                 val = (jj >= 0 && jj < n) ? g[jj] : 0.0;
             }
+            acc = acc + w[mi] * val;
+        }
+        out[j] = acc;
+    }
+}
+
+// ---- NEXT row N3: odd stencil width, per-point displacement (the paper's own section-5 benchmark kernel) -------
+// PAPER.md:86-89 eq (6): for odd q the stencil stays centred on the grid point,
+//   f(x_j + alpha) = sum_{i=j-(q-1)/2}^{j+(q-1)/2} l_i(alpha) f(x_i),   |alpha| < dx,
+// with l_m the Lagrange basis on the integer nodes m = -(q-1)/2 .. (q-1)/2 evaluated at alpha (in cells).
+// the displacement may be a function of all six coordinates ("random shifts alpha/dx in [-1,1]").
+void lagrange_weights_odd(int q, double alpha, double* w) {
+    const int h = (q - 1) / 2;
+    for (int mi = 0; mi < q; ++mi) {
+        const int m = mi - h;
+        double num = 1.0, den = 1.0;
+        for (int ni = 0; ni < q; ++ni) {
+            const int n = ni - h;
+            if (n == m) continue;
+            num = num * (alpha - (double)n);
+            den = den * (double)(m - n);
+        }
+        w[mi] = num / den;
+    }
+}
+
+// out[j] = sum_m l_m(alpha[j]) g[j+m]; g periodic (x dims) or zero outside [0,n) (v dims).
+void pencil_update_pointwise(int n, int q, bool periodic, const double* g, const double* alpha, double* out) {
+    const int h = (q - 1) / 2;
+    double w[kMaxQ];
+    for (int j = 0; j < n; ++j) {
+        lagrange_weights_odd(q, alpha[j], w);
+        double acc = 0.0;
+        for (int mi = 0; mi < q; ++mi) {
+            const long long jj = (long long)j + (long long)(mi - h);
+            double val;
+            if (periodic) val = g[((jj % n) + n) % n];
+            else val = (jj >= 0 && jj < n) ? g[jj] : 0.0;
             acc = acc + w[mi] * val;
         }
         out[j] = acc;
@@ -263,6 +303,43 @@ int oracle_strang_step(const int32_t* n, const double* lo, const double* dx, int
         if ((rc = oracle_rotate(n, lo, dx, degree, f, f, B, dt))) return rc;
     for (int d = 0; d < 3; ++d)
         if ((rc = oracle_advect(n, lo, dx, degree, f, f, d, nullptr, half))) return rc;
+    return 0;
+}
+
+int oracle_lagrange_weights_odd(int q, double alpha, double* w) {
+    if (q < 1 || q > kMaxQ || !(q & 1) || !w) return -1;
+    lagrange_weights_odd(q, alpha, w);
+    return 0;
+}
+
+// Sweep along `dim` with one displacement per POINT: alpha has the shape and layout of f (in cells).
+int oracle_sweep_pointwise(const int32_t* n, const double* f_in, double* f_out, int dim, const double* alpha, int q) {
+    if (!n || !f_in || !f_out || !alpha || dim < 0 || dim > 5 || q < 1 || q > kMaxQ || !(q & 1)) return -1;
+    long long stride[6];
+    stride[5] = 1;
+    for (int d = 4; d >= 0; --d) stride[d] = stride[d + 1] * n[d + 1];
+    const int nd = n[dim];
+    const bool periodic = dim < 3;
+    const long long npencil = total_points(n) / nd;
+#pragma omp parallel
+    {
+        std::vector<double> g(nd), a(nd), o(nd);
+#pragma omp for schedule(static)
+        for (long long p = 0; p < npencil; ++p) {
+            long long rem = p, base = 0;
+            for (int d = 5; d >= 0; --d) {
+                if (d == dim) continue;
+                base += (rem % n[d]) * stride[d];
+                rem /= n[d];
+            }
+            for (int j = 0; j < nd; ++j) {
+                g[j] = f_in[base + (long long)j * stride[dim]];
+                a[j] = alpha[base + (long long)j * stride[dim]];
+            }
+            pencil_update_pointwise(nd, q, periodic, g.data(), a.data(), o.data());
+            for (int j = 0; j < nd; ++j) f_out[base + (long long)j * stride[dim]] = o[j];
+        }
+    }
     return 0;
 }
 
