@@ -181,7 +181,31 @@ C4 = _mk("C4", (32,) * 6, FOUR_PI, 6.0, degree=7, dt=0.1, seed=1004, noise_amp=1
 C5 = _mk("C5", (48, 48, 48, 32, 32, 32), FOUR_PI, 6.0, degree=9, dt=0.05, seed=1005, noise_amp=1e-4,
          kind="maxwell_xyz", B=(0.0, 0.0, 1.0))
 
-CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5)}
+#: The paper's own section-5 benchmark grid: 37 points per dim, odd stencil widths 3/5/7/9, random
+#: per-point displacements alpha/dx in [-1, 1] (see random_shifts).  degree here is only the default even-q context.
+P37 = _mk("P37", (37,) * 6, FOUR_PI, 6.0, degree=7, dt=0.05, seed=1037, noise_amp=1e-3, kind="maxwell_x1")
+
+CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5, P37)}
+
+
+def random_shifts(shape: Sequence[int], seed: int, device="cpu", whole_cells: bool = False,
+                  slab_bytes: int = 1 << 29) -> torch.Tensor:
+    """Per-point displacements in cells for the paper's benchmark: alpha = 2 u(seed + lin) - 1 in [-1, 1) with the
+    same counter-based generator as the noise (bit-identical on CPU and CUDA); whole_cells=True rounds them to
+    {-1, 0, 1} (the exact-permutation test)."""
+    shape = tuple(int(v) for v in shape)
+    out = torch.empty(shape, dtype=torch.float64, device=device)
+    flat = out.view(-1)
+    total = flat.numel()
+    step = max(1, slab_bytes // 8)
+    for i0 in range(0, total, step):
+        i1 = min(total, i0 + step)
+        lin = torch.arange(i0, i1, dtype=torch.int64, device=device)
+        a = uniform_torch(seed, lin) * 2.0 - 1.0
+        if whole_cells:
+            a = torch.round(a)
+        flat[i0:i1] = a
+    return out
 
 
 def sample_pencils(npencil: int, count: int, seed: int) -> np.ndarray:

@@ -127,6 +127,18 @@ BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);
 
+/* ---- odd stencil width, one displacement per point ------------------------------------------
+ * PAPER.md:86-89 eq (6): for odd q the stencil stays centred on the grid point,
+ *     f_out[p, j] = sum_{m=-(q-1)/2..(q-1)/2} l_m(alpha[p, j]) * f_in[p, j + m]        (periodic in x, zero fill in v)
+ * with l_m the Lagrange basis on the integer nodes m evaluated at alpha (in cells; the paper assumes |alpha| < 1,
+ * PAPER.md:84).  alpha_cells is a DEVICE array with the shape and layout of f: "the most general way to define the
+ * interpolation shift is as a function of the full phase space" -- this is the kernel of the paper's
+ * own section-5 benchmark (random alpha/dx in [-1,1], widths 3/5/7/9, 37^6 points).  A sweep moves
+ * 24 B/point.  q in {3,5,7,9}; extents of `dim` in {8,16,32,37} (else BSL6D_EUNSUPPORTED).  f_in == f_out is legal;
+ * alpha_cells must not overlap f_out. */
+BSL6D_API int bsl6d_advect_pointwise(bsl6d_ctx* ctx, const double* f_in, double* f_out, int dim,
+                           const double* alpha_cells, int q, void* stream);
+
 /* ---- field step: the self-consistent electric field ------------------------------------------
  * PAPER.md:44-48 eq (2): rho_c = q (int f dv - n0), -Laplace(phi) = rho_c, E = -grad(phi), solved pseudo-spectrally on
  * the periodic x grid; eq (11): the adiabatic-electron closure (n0 q^2/T_e) phi = rho_c.

@@ -20,6 +20,7 @@ SYMBOLS = (
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
+    "bsl6d_advect_pointwise",
 )
 
 OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
@@ -79,6 +80,7 @@ def load_library() -> C.CDLL:
     lib.bsl6d_advect_seq.argtypes = [vp, dp, dp, C.POINTER(Sweep), C.c_int, vp]
     lib.bsl6d_seq_passes.argtypes = [vp, C.POINTER(Sweep), C.c_int]
     lib.bsl6d_set_fusion.argtypes = [vp, C.c_int]
+    lib.bsl6d_advect_pointwise.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, vp]
     lib.bsl6d_field_poisson.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
     lib.bsl6d_field_adiabatic.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
     lib.bsl6d_vp_step.argtypes = [vp, dp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, C.c_int,
@@ -219,6 +221,13 @@ class Context:
         if rc < 0:
             self._check(rc, "bsl6d_set_fusion")
         return rc
+
+    def advect_pointwise(self, f_in, f_out, dim: int, alpha_cells, q: int, stream=None):
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out"); self._shape_ok(alpha_cells, "alpha_cells")
+        self._check(self._lib.bsl6d_advect_pointwise(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"),
+                                                     int(dim), _dev_ptr(alpha_cells, "alpha_cells"), int(q),
+                                                     _stream(stream)), "bsl6d_advect_pointwise")
+        return f_out
 
     def _E3(self, E):
         nx = self.n[0] * self.n[1] * self.n[2]

@@ -13,6 +13,7 @@
 #include "field_kernels.cuh"
 #include "fused_api.h"
 #include "fused_kernels.cuh"
+#include "pointwise_kernels.cuh"
 #include "sweep_kernels.cuh"
 
 using bsl6d::SweepArgs;
@@ -740,6 +741,52 @@ int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     c->fusion = enable ? 1 : 0;
     c->fuse_all = enable == 2 ? 1 : 0;
     return old;
+}
+
+int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const double* alpha_cells,
+                           int q, void* stream) {
+    if (!c || !f_in || !f_out || !alpha_cells || dim < 0 || dim > 5) return BSL6D_EINVAL;
+    if (q < 1 || !(q & 1)) return BSL6D_EINVAL;
+    if (partial_overlap(c, f_in, f_out)) return BSL6D_EALIAS;
+    if (alpha_cells == f_out || partial_overlap(c, alpha_cells, f_out)) return BSL6D_EALIAS;
+    const int32_t* n = c->g.n;
+    size_t inner = 1, outer = 1;
+    for (int d = dim + 1; d < 6; ++d) inner *= (size_t)n[d];
+    for (int d = 0; d < dim; ++d) outer *= (size_t)n[d];
+    if (inner * outer > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
+    bsl6d::PointwiseChoice pc;
+    if (!bsl6d::pointwise_lookup(n[dim], q, dim < 3, inner == 1, pc)) return BSL6D_EUNSUPPORTED;
+    bsl6d::PointwiseArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.in = f_in;
+    a.out = f_out;
+    a.alpha = alpha_cells;
+    a.inner = (uint32_t)inner;
+    a.outer = (uint32_t)outer;
+    unsigned grid;
+    if (pc.unit) {
+        grid = (unsigned)((outer + (size_t)pc.threads - 1) / (size_t)pc.threads);
+    } else {
+        const uint64_t lim = inner < (uint64_t)pc.threads ? inner : (uint64_t)pc.threads;
+        a.ti_log2 = ceil_pow2_log2(lim);
+        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)pc.threads / TI;
+        a.nib = (uint32_t)((inner + TI - 1) / TI);
+        const uint64_t nbo = (outer + TO - 1) / TO;
+        if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+        grid = (unsigned)((uint64_t)a.nib * nbo);
+    }
+    cudaError_t e;
+    if (pc.smem > 48 * 1024) {
+        e = cudaFuncSetAttribute(pc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pc.smem);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+    void* args[] = {(void*)&a};
+    e = cudaLaunchKernel(pc.fn, dim3(grid), dim3(pc.threads), args, pc.smem, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
 }
 
 int bsl6d_field_poisson(bsl6d_ctx* c, const double* rho, double rho_fac, double e_fac, double* const E[3],

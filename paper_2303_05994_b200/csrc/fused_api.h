@@ -19,3 +19,14 @@ bool fused_lookup_q8(int na, int nb, bool pa, bool pb, int pattern, FusedChoice&
 bool fused_lookup_q10(int na, int nb, bool pa, bool pb, int pattern, FusedChoice& out);
 
 }  // namespace bsl6d
+
+// ---- pointwise (odd q, per-point displacement) kernels, bsl6d_pointwise.cu -------------------------------------
+namespace bsl6d {
+struct PointwiseChoice {
+    const void* fn;        // __global__ void (*)(PointwiseArgs)
+    int threads;
+    size_t smem;
+    int unit;              // 1: unit-stride kernel (block = `threads` pencils)
+};
+bool pointwise_lookup(int n, int q, bool periodic, bool unit_stride, PointwiseChoice& out);
+}  // namespace bsl6d

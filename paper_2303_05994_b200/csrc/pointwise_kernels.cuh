@@ -1,0 +1,155 @@
+// pointwise_kernels.cuh -- SURVEY.md 8(f) N3: odd stencil width with one displacement per POINT.
+//
+// PAPER.md:86-89 eq (6): for odd q the stencil stays centred on the grid point,
+//     f(x_j + alpha) = sum_{m=-h..h} l_m(alpha) f(x_{j+m}),   h = (q-1)/2,   |alpha| < dx,
+// and PAPER.md:100, 194, 244: the displacement may depend on all six coordinates -- the paper's own section-5
+// benchmark runs exactly this ("random shifts alpha/dx in [-1,1]", widths 3, 5, 7, 9, 37^6 points).
+// alpha is a full-size array in cells, so a sweep moves 24 B/point (f in, alpha in, f out) and the weights are
+// evaluated per point (5q flops + q FMAs).  As in sweep_kernels.cuh one thread owns one pencil and keeps it in
+// registers; because there is no integer part k here, every stencil index -- wrap or zero fill included -- is a
+// compile-time constant.  All loads of a pencil precede its stores => f_in == f_out is legal (alpha must not alias).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace bsl6d {
+
+template <int Q>
+struct OddDen {
+    double r[Q];
+    constexpr OddDen() : r() {
+        for (int i = 0; i < Q; ++i) {
+            double d = 1.0;
+            for (int j = 0; j < Q; ++j)
+                if (j != i) d *= (double)(i - j);
+            r[i] = 1.0 / d;
+        }
+    }
+};
+
+// l_m(alpha) on nodes m = i - H, i = 0..Q-1.  Prefix/suffix products (3Q multiplies) times compile-time reciprocal
+// denominators; a whole-cell alpha in [-H, H] is mapped to the exact unit vector (reading S11 carried over), so that
+// whole-cell displacements stay exact permutations.
+template <int Q>
+__device__ __forceinline__ void lagrange_weights_odd(double alpha, double (&w)[Q]) {
+    constexpr OddDen<Q> den{};
+    constexpr int H = (Q - 1) / 2;
+    double d[Q], pre[Q], suf[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) d[i] = alpha - (double)(i - H);
+    pre[0] = 1.0;
+#pragma unroll
+    for (int i = 1; i < Q; ++i) pre[i] = pre[i - 1] * d[i - 1];
+    suf[Q - 1] = 1.0;
+#pragma unroll
+    for (int i = Q - 2; i >= 0; --i) suf[i] = suf[i + 1] * d[i + 1];
+    bool hit = false;
+#pragma unroll
+    for (int i = 0; i < Q; ++i) hit = hit || (d[i] == 0.0);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+        double v = (pre[i] * suf[i]) * den.r[i];
+        if (hit) v = (d[i] == 0.0) ? 1.0 : 0.0;
+        w[i] = v;
+    }
+}
+
+struct PointwiseArgs {
+    const double* in;
+    double* out;
+    const double* alpha;   // same shape and layout as f, displacement in cells
+    uint32_t inner, outer; // as in SweepArgs
+    uint32_t ti_log2, nib;
+};
+
+template <int N, int Q, bool PERIODIC>
+__device__ __forceinline__ double stencil_at(const double (&u)[N], const double (&w)[Q], int j) {
+    constexpr int H = (Q - 1) / 2;
+    double acc = 0.0;
+    bool first = true;
+#pragma unroll
+    for (int m = 0; m < Q; ++m) {
+        const int jj = j + m - H;
+        double v;
+        if (PERIODIC) v = u[((jj % N) + N) % N];
+        else {
+            if (jj < 0 || jj >= N) continue;              // zero extension: the term vanishes
+            v = u[jj];
+        }
+        acc = first ? w[m] * v : fma(w[m], v, acc);
+        first = false;
+    }
+    return acc;
+}
+
+// strided dims (inner > 1): lanes along `inner`
+template <int N, int Q, bool PERIODIC, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB) pointwise_strided_kernel(const PointwiseArgs a) {
+    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
+    const uint32_t bo = blockIdx.x / a.nib;
+    const uint32_t bi = blockIdx.x - bo * a.nib;
+    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
+    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
+    if (i >= a.inner || o >= a.outer) return;
+    const size_t stride = a.inner;
+    const size_t base = (size_t)o * N * stride + i;
+    const double* __restrict__ pin = a.in + base;
+    const double* __restrict__ pal = a.alpha + base;
+    double* pout = a.out + base;
+    double u[N];
+#pragma unroll
+    for (int t = 0; t < N; ++t) u[t] = __ldcs(pin + (size_t)t * stride);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double w[Q];
+        lagrange_weights_odd<Q>(__ldcs(pal + (size_t)j * stride), w);
+        __stcs(pout + (size_t)j * stride, stencil_at<N, Q, PERIODIC>(u, w, j));
+    }
+}
+
+// unit-stride dim (inner == 1, always a v dim): T pencils per block, f and alpha transposed through two padded
+// shared-memory tiles; results overwrite the alpha tile (alpha_j is consumed when out_j is produced).
+template <int N, int Q, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB) pointwise_unit_kernel(const PointwiseArgs a) {
+    extern __shared__ double tiles[];                      // 2 x T x (N+1)
+    constexpr int LD = N + 1;
+    double* tf = tiles;
+    double* ta = tiles + T * LD;
+    const size_t p0 = (size_t)blockIdx.x * T;
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    const uint32_t nelem = np * N;
+    const double* __restrict__ pin = a.in + p0 * N;
+    const double* __restrict__ pal = a.alpha + p0 * N;
+    double* pout = a.out + p0 * N;
+#pragma unroll
+    for (int it = 0; it < N; ++it) {
+        const uint32_t e = it * T + threadIdx.x;
+        if (e < nelem) {
+            const uint32_t s = (e / N) * LD + (e % N);
+            tf[s] = __ldcs(pin + e);
+            ta[s] = __ldcs(pal + e);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < np) {
+        const double* rowf = tf + threadIdx.x * LD;
+        double* rowa = ta + threadIdx.x * LD;
+        double u[N];
+#pragma unroll
+        for (int t = 0; t < N; ++t) u[t] = rowf[t];
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+            double w[Q];
+            lagrange_weights_odd<Q>(rowa[j], w);
+            rowa[j] = stencil_at<N, Q, false>(u, w, j);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < N; ++it) {
+        const uint32_t e = it * T + threadIdx.x;
+        if (e < nelem) __stcs(pout + e, ta[(e / N) * LD + (e % N)]);
+    }
+}
+
+}  // namespace bsl6d

@@ -1,0 +1,124 @@
+"""Odd-q / per-point-displacement sweep on the GPU against the oracle."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import bsl6d_workloads as wl
+import oracle
+import paper_2303_05994_b200 as bsl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+def _need(gb=0.0):
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    if gb and torch.cuda.mem_get_info()[0] < gb * 2 ** 30:
+        pytest.skip(f"needs {gb} GiB of free device memory")
+
+
+def _ctx(n):
+    return bsl.create(n, (0.0,) * 3 + (-6.0,) * 3, (1.0,) * 6, 7)
+
+
+GRIDS = [(8, 16, 32, 37, 8, 16), (37, 8, 8, 16, 32, 37), (16, 37, 8, 8, 37, 32), (32, 8, 37, 8, 16, 8)]
+
+
+@pytest.mark.parametrize("n", GRIDS)
+@pytest.mark.parametrize("q", (3, 5, 7, 9))
+def test_every_dim_random_shifts(n, q):
+    _need()
+    rng = np.random.default_rng(q)
+    f = rng.random(n)
+    alpha = wl.random_shifts(n, 77 + q).numpy()
+    fd, ad = torch.from_numpy(f).cuda(), torch.from_numpy(alpha).cuda()
+    out = torch.empty_like(fd)
+    with _ctx(n) as ctx:
+        for dim in range(6):
+            ctx.advect_pointwise(fd, out, dim, ad, q)
+            ref = oracle.sweep_pointwise(f, dim, alpha, q)
+            err = np.max(np.abs(out.cpu().numpy() - ref)) / np.max(np.abs(ref))
+            assert err <= TOL, (dim, err)
+        inplace = fd.clone()
+        ctx.advect_pointwise(inplace, inplace, 2, ad, q)     # in place
+        assert torch.equal(inplace, ctx.advect_pointwise(fd, out, 2, ad, q))
+        assert ctx.launch_count() == 8
+
+
+@pytest.mark.parametrize("q", (3, 9))
+def test_whole_cell_shifts_are_bit_exact(q):
+    _need()
+    n = (37, 8, 16, 32, 8, 37)
+    f = np.random.default_rng(1).random(n)
+    alpha = wl.random_shifts(n, 5, whole_cells=True).numpy()
+    assert set(np.unique(alpha)) == {-1.0, 0.0, 1.0}
+    fd, ad = torch.from_numpy(f).cuda(), torch.from_numpy(alpha).cuda()
+    out = torch.empty_like(fd)
+    with _ctx(n) as ctx:
+        for dim in range(6):
+            ctx.advect_pointwise(fd, out, dim, ad, q)
+            assert np.array_equal(out.cpu().numpy(), oracle.sweep_pointwise(f, dim, alpha, q)), dim
+    # and the expected value needs no oracle at all: out[j] = in[j + alpha_j] (periodic dim 0)
+    with _ctx(n) as ctx:
+        got = ctx.advect_pointwise(fd, out, 0, ad, q).cpu().numpy()
+    j = np.arange(37).reshape(37, 1, 1, 1, 1, 1)
+    src = (j + alpha.astype(np.int64)) % 37
+    assert np.array_equal(got, np.take_along_axis(f, src, axis=0))
+
+
+def test_generator_cpu_equals_cuda():
+    _need()
+    a = wl.random_shifts((5, 4, 3, 2, 3, 4), 9)
+    assert torch.equal(a, wl.random_shifts((5, 4, 3, 2, 3, 4), 9, device="cuda").cpu())
+    assert float(a.min()) >= -1.0 and float(a.max()) < 1.0
+
+
+def test_error_codes():
+    _need()
+    n = (8, 8, 8, 8, 8, 12)
+    f = torch.zeros(n, dtype=torch.float64, device="cuda")
+    a = torch.zeros_like(f)
+    with _ctx(n) as ctx:
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_pointwise(f, f, 0, a, 4)              # even width
+        assert e.value.code == bsl.EINVAL
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_pointwise(f, f, 0, f, 3)              # alpha aliases the output
+        assert e.value.code == bsl.EALIAS
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_pointwise(f, f, 5, a, 3)              # extent 12 has no kernel
+        assert e.value.code == bsl.EUNSUPPORTED
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.advect_pointwise(f, f, 0, a, 11)             # width 11 has no kernel
+        assert e.value.code == bsl.EUNSUPPORTED
+        assert ctx.launch_count() == 0
+
+
+def test_paper_benchmark_grid_full_size_sampled():
+    """37^6 (20.5 GB per array, three arrays), width 7, every direction: oracle on sampled pencils of f and alpha."""
+    _need(70)
+    w = wl.P37
+    f = w.make_f("cuda")
+    alpha = wl.random_shifts(w.n, w.seed + 1, device="cuda")
+    out = torch.empty_like(f)
+    rng = np.random.default_rng(2037)
+    P, N = 1024, 37
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for dim in range(6):
+            outer = int(np.prod(w.n[:dim], dtype=np.int64))
+            inner = int(np.prod(w.n[dim + 1:], dtype=np.int64))
+            o = torch.from_numpy(rng.integers(0, outer, P)).cuda()
+            i = torch.from_numpy(rng.integers(0, inner, P)).cuda()
+            ctx.advect_pointwise(f, out, dim, alpha, 7)
+            g = lambda t: t.view(outer, N, inner)[o, :, i].cpu().numpy()          # (P, N)
+            gi, ga, go = g(f), g(alpha), g(out)
+            if dim < 3:      # mini-grid: swept dim at position 0 (periodic), samples at position 3
+                ref = oracle.sweep_pointwise(np.ascontiguousarray(gi.T).reshape(N, 1, 1, P, 1, 1), 0,
+                                             np.ascontiguousarray(ga.T).reshape(N, 1, 1, P, 1, 1), 7).reshape(N, P).T
+            else:            # swept dim at position 3 (zero-extended), samples at position 0
+                ref = oracle.sweep_pointwise(gi.reshape(P, 1, 1, N, 1, 1), 3, ga.reshape(P, 1, 1, N, 1, 1), 7).reshape(P, N)
+            err = np.max(np.abs(go - ref)) / np.max(np.abs(ref))
+            assert err <= TOL, (dim, err)
