@@ -50,6 +50,9 @@ def parse_args():
     p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     p.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     p.add_argument("--no-fused", action="store_true", help="skip the fused-pass variant of the step")
+    p.add_argument("--paper-benchmark", action="store_true",
+                   help="instead of the contract step: the paper's own section-5 benchmark (37^6, random per-point "
+                        "shifts, odd widths 3/5/7/9, every direction) through bsl6d_advect_pointwise")
     return p.parse_args()
 
 
@@ -462,8 +465,64 @@ def run_ours(args, w):
         dist.destroy_process_group()
 
 
+def run_paper_benchmark(args):
+    """one 1-D interpolation per direction on 37^6 points, random alpha/dx in [-1,1] per
+    point, odd stencil widths.  Reports, per width and direction, the time and GB/s in the paper's convention
+    (16 B/point: f read + f written, eq (8)) and with the alpha array counted (24 B/point)."""
+    import torch
+    import bsl6d_workloads as wl
+    import paper_2303_05994_b200 as bsl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    torch.cuda.set_device(0)
+    bsl.load_library()
+    w = wl.P37
+    f = w.make_f("cuda")
+    alpha = wl.random_shifts(w.n, w.seed + 1, device="cuda")
+    out = torch.empty_like(f)
+    ctx = bsl.create(w.n, w.lo, w.dx, w.degree)
+    stream = torch.cuda.current_stream()
+    K = max(1, args.steps)
+    res = {}
+    clocks = ClockSampler(0)
+    clocks.start()
+    for q in (3, 5, 7, 9):
+        row = {}
+        for dim, nm in enumerate(("x1", "x2", "x3", "v1", "v2", "v3")):
+            for _ in range(max(args.warmup, 1)):
+                ctx.advect_pointwise(f, out, dim, alpha, q)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(K):
+                ctx.advect_pointwise(f, out, dim, alpha, q)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / K
+            row[nm] = {"ms": ms, "GB/s_16B_per_point": 16 * w.npts / ms / 1e6, "GB/s_24B_per_point": 24 * w.npts / ms / 1e6,
+                       "Gpoint-updates/s": w.npts / ms / 1e6}
+        res[f"q{q}"] = row
+    clk = clocks.stop()
+    ctx.destroy()
+    peak, peak_src = peaks()
+    allv = [v["GB/s_24B_per_point"] for r in res.values() for v in r.values()]
+    line = {"metric": "paper section-5 benchmark: 1-D Lagrange interpolation per direction, 37^6 fp64 points, random "
+                      "per-point shifts in [-1,1] cells, odd widths (GB/s; paper's convention 16 B/point)",
+            "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": max(args.warmup, 1), "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "P37 37x37x37x37x37x37 (PAPER.md:194, 244), alpha array resident (24 B/point moved)"},
+            "value": float(np.mean([v["GB/s_16B_per_point"] for r in res.values() for v in r.values()])),
+            "mean_GB/s_24B": float(np.mean(allv)), "min_GB/s_24B": float(min(allv)), "max_GB/s_24B": float(max(allv)),
+            "peak": peak, "peak_source": peak_src, "frac_of_peak_24B": float(np.mean(allv)) / peak,
+            "paper_context": {"V100": "almost 500 GB/s", "Xeon Gold 6148 node": "around 100 GB/s", "cite": "PAPER.md:11"},
+            "clocks": clk, "per_width": res}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
+    if args.paper_benchmark:
+        run_paper_benchmark(args)
+        return
     import bsl6d_workloads as wl
     w = wl.CONFIGS[args.workload]
     if args.impl == "reference":

@@ -767,13 +767,8 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
     if (pc.unit) {
         grid = (unsigned)((outer + (size_t)pc.threads - 1) / (size_t)pc.threads);
     } else {
-        const uint64_t lim = inner < (uint64_t)pc.threads ? inner : (uint64_t)pc.threads;
-        a.ti_log2 = ceil_pow2_log2(lim);
-        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)pc.threads / TI;
-        a.nib = (uint32_t)((inner + TI - 1) / TI);
-        const uint64_t nbo = (outer + TO - 1) / TO;
-        if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
-        grid = (unsigned)((uint64_t)a.nib * nbo);
+        a.npencil = (uint32_t)(inner * outer);
+        grid = (unsigned)((inner * outer + (size_t)pc.threads - 1) / (size_t)pc.threads);
     }
     cudaError_t e;
     if (pc.smem > 48 * 1024) {

@@ -7,7 +7,7 @@ namespace {
 
 template <int N, int Q>
 constexpr int pw_minblocks() {
-    constexpr int est = 2 * N + 6 * Q + 40;                 // registers a thread wants (pencil + weight scratch)
+    constexpr int est = 4 * N + 6 * Q + 40;                 // registers a thread wants (pencil + shifts + weight scratch)
     return est <= 128 ? 4 : (est <= 170 ? 3 : 2);
 }
 

@@ -43,14 +43,11 @@ __device__ __forceinline__ void lagrange_weights_odd(double alpha, double (&w)[Q
     suf[Q - 1] = 1.0;
 #pragma unroll
     for (int i = Q - 2; i >= 0; --i) suf[i] = suf[i + 1] * d[i + 1];
-    bool hit = false;
 #pragma unroll
-    for (int i = 0; i < Q; ++i) hit = hit || (d[i] == 0.0);
+    for (int i = 0; i < Q; ++i) w[i] = (pre[i] * suf[i]) * den.r[i];
+    if (alpha == rint(alpha) && fabs(alpha) <= (double)H) {       // whole-cell displacement: rare, exact
 #pragma unroll
-    for (int i = 0; i < Q; ++i) {
-        double v = (pre[i] * suf[i]) * den.r[i];
-        if (hit) v = (d[i] == 0.0) ? 1.0 : 0.0;
-        w[i] = v;
+        for (int i = 0; i < Q; ++i) w[i] = (d[i] == 0.0) ? 1.0 : 0.0;
     }
 }
 
@@ -59,7 +56,7 @@ struct PointwiseArgs {
     double* out;
     const double* alpha;   // same shape and layout as f, displacement in cells
     uint32_t inner, outer; // as in SweepArgs
-    uint32_t ti_log2, nib;
+    uint32_t npencil;      // inner * outer
 };
 
 template <int N, int Q, bool PERIODIC>
@@ -82,27 +79,29 @@ __device__ __forceinline__ double stencil_at(const double (&u)[N], const double 
     return acc;
 }
 
-// strided dims (inner > 1): lanes along `inner`
+// strided dims (inner > 1)
 template <int N, int Q, bool PERIODIC, int T, int MINB>
 __global__ void __launch_bounds__(T, MINB) pointwise_strided_kernel(const PointwiseArgs a) {
-    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
-    const uint32_t bo = blockIdx.x / a.nib;
-    const uint32_t bi = blockIdx.x - bo * a.nib;
-    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
-    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
-    if (i >= a.inner || o >= a.outer) return;
+    // lanes run along the flattened pencil index (o, i): full lane use for any `inner` (37 is not a power of two)
+    const uint32_t p = blockIdx.x * T + threadIdx.x;
+    if (p >= a.npencil) return;
+    const uint32_t o = p / a.inner, i = p - o * a.inner;
     const size_t stride = a.inner;
     const size_t base = (size_t)o * N * stride + i;
     const double* __restrict__ pin = a.in + base;
     const double* __restrict__ pal = a.alpha + base;
     double* pout = a.out + base;
-    double u[N];
+    // every load of the pencil -- values and displacements -- is issued before the first store: 2N loads in flight
+    // per thread, and stores to f_out can never be ordered between them (f_out may alias f_in)
+    double u[N], al[N];
 #pragma unroll
     for (int t = 0; t < N; ++t) u[t] = __ldcs(pin + (size_t)t * stride);
 #pragma unroll
+    for (int t = 0; t < N; ++t) al[t] = __ldcs(pal + (size_t)t * stride);
+#pragma unroll
     for (int j = 0; j < N; ++j) {
         double w[Q];
-        lagrange_weights_odd<Q>(__ldcs(pal + (size_t)j * stride), w);
+        lagrange_weights_odd<Q>(al[j], w);
         __stcs(pout + (size_t)j * stride, stencil_at<N, Q, PERIODIC>(u, w, j));
     }
 }
