@@ -140,6 +140,34 @@ bool unit_lookup(int n, int q, KernelChoice& c) {
     }
 }
 
+template <int T>
+const void* generic_by_q(int q) {
+    switch (q) {
+        case 2: return (const void*)bsl6d::sweep_generic_kernel<2, T>;
+        case 4: return (const void*)bsl6d::sweep_generic_kernel<4, T>;
+        case 6: return (const void*)bsl6d::sweep_generic_kernel<6, T>;
+        case 8: return (const void*)bsl6d::sweep_generic_kernel<8, T>;
+        case 10: return (const void*)bsl6d::sweep_generic_kernel<10, T>;
+        case 12: return (const void*)bsl6d::sweep_generic_kernel<12, T>;
+        default: return nullptr;
+    }
+}
+const void* generic_fn(int q, int T) { return T == 64 ? generic_by_q<64>(q) : generic_by_q<32>(q); }
+
+template <int T>
+const void* generic_unit_by_q(int q) {
+    switch (q) {
+        case 2: return (const void*)bsl6d::sweep_generic_unit_kernel<2, T>;
+        case 4: return (const void*)bsl6d::sweep_generic_unit_kernel<4, T>;
+        case 6: return (const void*)bsl6d::sweep_generic_unit_kernel<6, T>;
+        case 8: return (const void*)bsl6d::sweep_generic_unit_kernel<8, T>;
+        case 10: return (const void*)bsl6d::sweep_generic_unit_kernel<10, T>;
+        case 12: return (const void*)bsl6d::sweep_generic_unit_kernel<12, T>;
+        default: return nullptr;
+    }
+}
+const void* generic_unit_fn(int q, int T) { return T == 64 ? generic_unit_by_q<64>(q) : generic_unit_by_q<32>(q); }
+
 // Which kernel serves a sweep along `dim`?  (Also used by bsl6d_kernel_name.)
 int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     const int n = c->g.n[dim];
@@ -150,12 +178,13 @@ int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     if (inner == 1) ok = !periodic && unit_lookup(n, c->q, k);
     else ok = periodic ? strided_lookup<true>(n, c->q, k) : strided_lookup<false>(n, c->q, k);
     if (ok) return BSL6D_OK;
-    // fallback: column staged in shared memory, n * T doubles
+    // fallback: pencils staged in shared memory: n * T doubles (strided), 2 * (n|1) * T doubles (unit stride)
     const size_t cap = 200 * 1024;
+    const size_t per_thread = ((inner == 1 && !periodic) ? 2 * (size_t)(n | 1) : (size_t)n) * sizeof(double);
     int T = 64;
-    if ((size_t)n * T * sizeof(double) > cap) T = 32;
-    if ((size_t)n * T * sizeof(double) > cap) return BSL6D_EUNSUPPORTED;
-    k = KernelChoice{nullptr, T, (size_t)n * T * sizeof(double), 2, T};
+    if (per_thread * T > cap) T = 32;
+    if (per_thread * T > cap) return BSL6D_EUNSUPPORTED;
+    k = KernelChoice{nullptr, T, per_thread * T, 2, T};
     return BSL6D_OK;
 }
 
@@ -257,17 +286,17 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
 
     cudaError_t e;
     if (kc.kind == 2) {
-        if (kc.gen_T == 64) {
-            e = cudaFuncSetAttribute(bsl6d::sweep_generic_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)kc.smem);
+        const void* gfn = (inner == 1 && dim >= 3) ? generic_unit_fn(c->q, kc.gen_T) : generic_fn(c->q, kc.gen_T);
+        if (!gfn) return BSL6D_EUNSUPPORTED;
+        if (kc.smem > 48 * 1024) {
+            e = cudaFuncSetAttribute(gfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kc.smem);
             if (e != cudaSuccess) return cuda_fail(c, e);
-            bsl6d::sweep_generic_kernel<64><<<grid, 64, kc.smem, stream>>>(a, c->q, dim < 3 ? 1 : 0);
-        } else {
-            e = cudaFuncSetAttribute(bsl6d::sweep_generic_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)kc.smem);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-            bsl6d::sweep_generic_kernel<32><<<grid, 32, kc.smem, stream>>>(a, c->q, dim < 3 ? 1 : 0);
         }
+        int per = dim < 3 ? 1 : 0;
+        void* gargs[] = {(void*)&a, (void*)&per};                  // the unit-stride kernel takes only `a`
+        grid = (unsigned)((inner * outer + (size_t)kc.gen_T - 1) / (size_t)kc.gen_T);
+        e = cudaLaunchKernel(gfn, dim3(grid), dim3(kc.gen_T), gargs, kc.smem, stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
     } else {
         if (kc.smem > 48 * 1024) {
             e = cudaFuncSetAttribute((const void*)kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kc.smem);

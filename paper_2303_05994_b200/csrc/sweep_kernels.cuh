@@ -239,54 +239,117 @@ __global__ void __launch_bounds__(T, MINB) sweep_unit_kernel(const SweepArgs a) 
     }
 }
 
-// ---- fallback for extents / widths without a specialised instance -------------------------------------------
-// One column per thread, staged in shared memory as tile[row * T + tid]; q loads per output.  Correct for any
-// n, any even q <= 12, both boundary kinds, inner >= 1; not tuned.
-template <int T>
-__global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int q, int periodic) {
+// ---- fallback for extents without a specialised instance (any n, even q <= 12) -------------------------------
+// One pencil per thread, lanes along the flattened pencil index (full lane use for any `inner`).  The column is
+// staged in shared memory as tile[row * T + tid] (all n loads in flight, and f_in == f_out stays legal), then a
+// register window of Q values slides along it: one shared-memory read and Q FMAs per output, the same
+// split_shift / lagrange_weights / fma order as the specialised kernels (so the numbers are bit-identical).
+template <int Q, int T>
+__global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int periodic) {
     extern __shared__ double tile[];                       // n * T
-    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
-    const uint32_t bo = blockIdx.x / a.nib;
-    const uint32_t bi = blockIdx.x - bo * a.nib;
-    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
-    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
-    if (i >= a.inner || o >= a.outer) return;
+    const uint32_t p = blockIdx.x * T + threadIdx.x;
+    if (p >= a.inner * a.outer) return;
+    const uint32_t o = p / a.inner, i = p - o * a.inner;
     const int n = (int)a.n;
     long long k;
     double theta;
     split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
     const size_t stride = a.inner;
     const size_t base = (size_t)o * n * stride + i;
-    for (int r = 0; r < n; ++r) tile[r * T + threadIdx.x] = __ldcs(a.in + base + (size_t)r * stride);
+    double* col = tile + threadIdx.x;
+#pragma unroll 8
+    for (int r = 0; r < n; ++r) col[r * T] = __ldcs(a.in + base + (size_t)r * stride);
 
-    double w[12];
-    {
-        // same product form as lagrange_weights<Q>, run-time q
-        const int mlo = 1 - q / 2;
-        for (int ii = 0; ii < q; ++ii) {
-            double num = 1.0, den = 1.0;
-            for (int jj = 0; jj < q; ++jj) {
-                if (jj == ii) continue;
-                num *= theta - (double)(mlo + jj);
-                den *= (double)(ii - jj);
-            }
-            w[ii] = num / den;
-        }
+    double w[Q];
+    lagrange_weights<Q>(theta, w);
+
+    // row of the first stencil node of output 0, then advanced by one per output
+    long long kk = k + (long long)(1 - Q / 2);
+    int row;
+    if (periodic) {
+        kk %= n;
+        if (kk < 0) kk += n;
+        row = (int)kk;
+    } else {
+        const long long lim = 2LL * n + 32;
+        kk = kk < -lim ? -lim : (kk > lim ? lim : kk);
+        row = (int)kk;
     }
-    long long kk = k + (long long)(1 - q / 2);             // first stencil row for j = 0
-    if (periodic) { kk %= n; if (kk < 0) kk += n; }
-    else { const long long lim = 2LL * n + 32; kk = kk < -lim ? -lim : (kk > lim ? lim : kk); }
+    auto fetch = [&](int r) -> double {
+        if (periodic) return col[r * T];
+        return (r >= 0 && r < n) ? col[r * T] : 0.0;
+    };
+    auto next = [&](int r) -> int {
+        ++r;
+        if (periodic && r >= n) r -= n;
+        return r;
+    };
+    double win[Q];
+#pragma unroll
+    for (int m = 0; m < Q - 1; ++m) {
+        win[m + 1] = fetch(row);                             // win[1..Q-1] primed; shifted down in the loop
+        row = next(row);
+    }
     for (int j = 0; j < n; ++j) {
-        double acc = 0.0;
-        for (int m = 0; m < q; ++m) {
-            long long r = kk + j + m;
-            double v;
-            if (periodic) { r %= n; v = tile[(int)r * T + threadIdx.x]; }
-            else v = (r >= 0 && r < n) ? tile[(int)r * T + threadIdx.x] : 0.0;
-            acc = (m == 0) ? w[0] * v : fma(w[m], v, acc);
-        }
+#pragma unroll
+        for (int m = 0; m < Q - 1; ++m) win[m] = win[m + 1];
+        win[Q - 1] = fetch(row);
+        row = next(row);
+        double acc = w[0] * win[0];
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], win[m], acc);
         __stcs(a.out + base + (size_t)j * stride, acc);
     }
+}
+
+// The same for the unit-stride dim (inner == 1; always a v dim => zero extension): a block owns T consecutive
+// pencils = one contiguous chunk, moved coalesced through two shared-memory tiles (input rows, output rows) with an
+// odd row pitch, so that "lane = pencil" accesses are conflict-free.
+template <int Q, int T>
+__global__ void __launch_bounds__(T) sweep_generic_unit_kernel(const SweepArgs a) {
+    extern __shared__ double tile[];                       // 2 * T * LD
+    const int n = (int)a.n;
+    const int LD = n | 1;
+    double* tin = tile;
+    double* tout = tile + (size_t)T * LD;
+    const size_t p0 = (size_t)blockIdx.x * T;
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    const uint32_t nelem = np * (uint32_t)n;
+    const double* __restrict__ pin = a.in + p0 * n;
+    double* pout = a.out + p0 * n;
+    for (uint32_t e = threadIdx.x; e < nelem; e += T) tin[(e / n) * LD + (e % n)] = __ldcs(pin + e);
+    __syncthreads();
+    if (threadIdx.x < np) {
+        long long k;
+        double theta;
+        split_shift(__ldg(a.src + src_offset(a.terms, (uint32_t)(p0 + threadIdx.x), 0u)), a.scale, k, theta);
+        double w[Q];
+        lagrange_weights<Q>(theta, w);
+        const long long lim = 2LL * n + 32;
+        long long kk = k + (long long)(1 - Q / 2);
+        kk = kk < -lim ? -lim : (kk > lim ? lim : kk);
+        int row = (int)kk;
+        const double* rin = tin + threadIdx.x * LD;
+        double* rout = tout + threadIdx.x * LD;
+        double win[Q];
+#pragma unroll
+        for (int m = 0; m < Q - 1; ++m) {
+            win[m + 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
+            ++row;
+        }
+        for (int j = 0; j < n; ++j) {
+#pragma unroll
+            for (int m = 0; m < Q - 1; ++m) win[m] = win[m + 1];
+            win[Q - 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
+            ++row;
+            double acc = w[0] * win[0];
+#pragma unroll
+            for (int m = 1; m < Q; ++m) acc = fma(w[m], win[m], acc);
+            rout[j] = acc;
+        }
+    }
+    __syncthreads();
+    for (uint32_t e = threadIdx.x; e < nelem; e += T) __stcs(pout + e, tout[(e / n) * LD + (e % n)]);
 }
 
 }  // namespace bsl6d

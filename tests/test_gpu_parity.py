@@ -113,6 +113,11 @@ GRIDS = [
     ((9, 3, 12, 6, 10, 14), 11),      # q=12 has no specialised instance -> generic everywhere
     ((8, 16, 32, 16, 32, 16), 3),     # q=4 instances
     ((3, 2, 2, 2, 3, 200), 7),        # long unit-stride pencils (fallback), tiny everything else
+    ((5, 3, 9, 1, 1, 1), 3),          # degenerate: x3 is periodic AND unit-stride (inner == 1) -> strided fallback
+    ((1, 1, 1, 7, 5, 11), 5),         # no x extent at all
+    ((13, 1, 1, 21, 1, 1), 1),        # 1D1V, linear interpolation (q = 2)
+    ((2, 1, 37, 1, 1, 40), 7),        # the paper's extent 37 (fallback for even q) + unit-stride fallback
+    ((37, 2, 2, 37, 2, 37), 7),       # 37 in strided periodic, strided zero and unit-stride position
 ]
 
 
