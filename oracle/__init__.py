@@ -47,6 +47,7 @@ def _load():
         lib.oracle_rotate.argtypes = [ip, dp, dp, C.c_int, dp, dp, dp, C.c_double]
         lib.oracle_density.argtypes = [ip, dp, dp, dp]
         lib.oracle_strang_step.argtypes = [ip, dp, dp, C.c_int, dp, dp, dp, dp, dp, C.c_double]
+        lib.oracle_rotation_plan.argtypes = [dp, C.c_double, C.POINTER(C.c_int), dp]
         lib.oracle_lagrange_weights_odd.argtypes = [C.c_int, C.c_double, dp]
         lib.oracle_sweep_pointwise.argtypes = [ip, dp, dp, C.c_int, dp, C.c_int]
         _lib = lib
@@ -160,6 +161,17 @@ def rotate(grid: Grid, degree: int, f_in: np.ndarray, B: Sequence[float], dt: fl
     Bc = (C.c_double * 3)(*[float(b) for b in B])
     _check(_load().oracle_rotate(n, lo, dx, degree, _dp(f_in), _dp(out), Bc, float(dt)), "rotate")
     return out
+
+
+def rotation_plan(B: Sequence[float], dt: float):
+    """[(axis, angle)] -- the coordinate-axis rotations rotate() applies, in order, for an oblique B (reading R1)."""
+    Bc = (C.c_double * 3)(*[float(b) for b in B])
+    axes = (C.c_int * 16)()
+    ang = (C.c_double * 16)()
+    cnt = _load().oracle_rotation_plan(Bc, float(dt), axes, ang)
+    if cnt < 0:
+        raise ValueError("rotation_plan wants B with at least two non-zero components")
+    return [(int(axes[i]), float(ang[i])) for i in range(cnt)]
 
 
 def density(grid: Grid, f: np.ndarray) -> np.ndarray:

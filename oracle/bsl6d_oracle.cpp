@@ -188,21 +188,56 @@ std::vector<double> nodes(const Grid& g, int d) {
 // B = (q/m) B0 has exactly one non-zero component c; (a,b,c) cyclic; theta = B_c * dt.
 //   f_new(v) = f_old(R(theta) v),  R = Sa(-tan(theta/2)) Sb(sin theta) Sa(-tan(theta/2)),
 // the backward foot of dV/dt = V x B (eq (3)).
-int rotate(const Grid& g, int q, const double* f_in, double* f_out, const double B[3], double dt) {
-    int c = -1;
-    for (int i = 0; i < 3; ++i) {
-        if (B[i] != 0.0) { if (c >= 0) return -3; c = i; }
-    }
-    const long long npts = total_points(g.n);
-    if (c < 0) { if (f_in != f_out) std::memcpy(f_out, f_in, sizeof(double) * npts); return 0; }
+// Rotation about ONE coordinate axis c by `theta` as three shears (BASELINE.json configs[3], reading S7):
+// (a,b,c) cyclic; foot displacement along v_a: -v_b*tan(theta/2); along v_b: +v_a*sin(theta); along v_a again.
+// Result: f_out(v) = f_in(R_c(theta) v), R_c the right-handed rotation about axis c.
+void rotate_axis(const Grid& g, int q, const double* f_in, double* f_out, int c, double theta) {
     const int a = (c + 1) % 3, b = (c + 2) % 3;
-    const double theta = B[c] * dt;
     const double t = std::tan(0.5 * theta), s = std::sin(theta);
     const std::vector<double> va = nodes(g, 3 + a), vb = nodes(g, 3 + b);
-    // foot displacement along v_a: -v_b*tan(theta/2);  along v_b: +v_a*sin(theta)
     sweep(g.n, f_in,  f_out, 3 + a, vb.data(), 1u << (3 + b), t / g.dx[3 + a], q);
     sweep(g.n, f_out, f_out, 3 + b, va.data(), 1u << (3 + a), -s / g.dx[3 + b], q);
     sweep(g.n, f_out, f_out, 3 + a, vb.data(), 1u << (3 + b), t / g.dx[3 + a], q);
+}
+
+// NEXT row N4 (oblique B): the axis-rotation sequence for a field B in general position (reading R1):
+// with b = B/|B| = (sin(vt)cos(ph), sin(vt)sin(ph), cos(vt)) and theta = |B| dt,
+//     R(b, theta) = Rz(ph) Ry(vt) Rz(theta) Ry(-vt) Rz(-ph),
+// and since (T_M f)(v) = f(M v) composes as T_A T_B = T_{BA}, the factors are APPLIED left to right:
+//     Rz(ph), Ry(vt), Rz(theta), Ry(-vt), Rz(-ph).
+// An axis rotation by more than pi/2 is applied in ceil(|angle| / (pi/2)) equal pieces (tan(piece/2) stays <= 1).
+// |theta| <= 2 pi is required (at most 4 + 4*2 = 12 entries... 16 reserved).
+int rotation_plan(const double B[3], double dt, int* axes, double* angles) {
+    const double bn = std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+    const double theta = bn * dt;
+    const double vt = std::acos(B[2] / bn);
+    const double ph = std::atan2(B[1], B[0]);
+    const int ax[5] = {2, 1, 2, 1, 2};
+    const double an[5] = {ph, vt, theta, -vt, -ph};
+    const double half_pi = 1.5707963267948966;
+    int cnt = 0;
+    for (int i = 0; i < 5; ++i) {
+        if (an[i] == 0.0) continue;
+        const int pieces = (int)std::ceil(std::fabs(an[i]) / half_pi);
+        for (int k = 0; k < pieces && cnt < 16; ++k) { axes[cnt] = ax[i]; angles[cnt++] = an[i] / (double)pieces; }
+    }
+    return cnt;
+}
+
+int rotate(const Grid& g, int q, const double* f_in, double* f_out, const double B[3], double dt) {
+    int c = -1, nz = 0;
+    for (int i = 0; i < 3; ++i)
+        if (B[i] != 0.0) { c = i; ++nz; }
+    const long long npts = total_points(g.n);
+    if (nz == 0) { if (f_in != f_out) std::memcpy(f_out, f_in, sizeof(double) * npts); return 0; }
+    if (nz == 1) { rotate_axis(g, q, f_in, f_out, c, B[c] * dt); return 0; }
+    int axes[16];
+    double angles[16];
+    if (std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]) * std::fabs(dt) > 6.283185307179586477) return -1;
+    const int cnt = rotation_plan(B, dt, axes, angles);
+    const double* cur = f_in;
+    for (int i = 0; i < cnt; ++i) { rotate_axis(g, q, cur, f_out, axes[i], angles[i]); cur = f_out; }
+    if (cnt == 0 && f_in != f_out) std::memcpy(f_out, f_in, sizeof(double) * npts);
     return 0;
 }
 
@@ -304,6 +339,15 @@ int oracle_strang_step(const int32_t* n, const double* lo, const double* dx, int
     for (int d = 0; d < 3; ++d)
         if ((rc = oracle_advect(n, lo, dx, degree, f, f, d, nullptr, half))) return rc;
     return 0;
+}
+
+// The (axis, angle) list rotate() applies for an oblique B (up to 16 entries); returns the count.
+int oracle_rotation_plan(const double* B, double dt, int* axes, double* angles) {
+    if (!B || !axes || !angles) return -1;
+    int nz = 0;
+    for (int i = 0; i < 3; ++i) nz += B[i] != 0.0;
+    if (nz < 2) return -1;
+    return rotation_plan(B, dt, axes, angles);
 }
 
 int oracle_lagrange_weights_odd(int q, double alpha, double* w) {

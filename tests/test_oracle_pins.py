@@ -365,11 +365,11 @@ def test_rotation_2pi_return():
     assert np.max(np.abs(f - f0)) > 0.1
 
 
-def test_rotate_rejects_oblique_B_and_identity_for_zero_B():
+def test_rotate_rejects_more_than_a_full_turn_about_an_oblique_axis_and_identity_for_zero_B():
     g = small_grid([1, 1, 1, 8, 8, 8])
     f = np.random.default_rng(0).random(g.n)
     with pytest.raises(ValueError):
-        oracle.rotate(g, 7, f, [0.1, 0.2, 0.0], 0.1)
+        oracle.rotate(g, 7, f, [3.0, 4.0, 0.0], 1.3)          # |B| dt = 6.5 > 2 pi (oblique B: tests/test_oracle_oblique.py)
     assert np.array_equal(oracle.rotate(g, 7, f, [0.0, 0.0, 0.0], 0.1), f)
 
 
