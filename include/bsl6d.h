@@ -52,7 +52,7 @@ enum {
     BSL6D_OK = 0,
     BSL6D_EINVAL = -1,        /* null pointer, bad extent / spacing / degree / dim / mask, non-finite dt */
     BSL6D_EALIAS = -2,        /* f_in and f_out overlap partially (exact aliasing f_in == f_out is legal) */
-    BSL6D_EUNSUPPORTED = -3,  /* B with more than one non-zero component; extent too large for on-chip staging */
+    BSL6D_EUNSUPPORTED = -3,  /* oblique B turning more than 2 pi; extent without a kernel / too large for on-chip staging */
     BSL6D_ECUDA = -4,         /* CUDA runtime failure; see bsl6d_last_cuda_error */
     BSL6D_ENOMEM = -5         /* host or device allocation failed */
 };
@@ -81,12 +81,16 @@ BSL6D_API int bsl6d_advect(bsl6d_ctx* ctx, const double* f_in, double* f_out, in
 BSL6D_API int bsl6d_advect_generic(bsl6d_ctx* ctx, const double* f_in, double* f_out, int dim,
                          const double* src, unsigned src_dim_mask, double scale, void* stream);
 
-/* Rotation of velocity space by the background field, dV/dt = V x B (eq (3)), as three velocity
- * shears (BASELINE.json configs[3], reading S7): with B (HOST, 3 doubles, = (q/m)*B0) along axis c,
- * (a,b,c) cyclic, theta = B[c]*dt:  shear v_a by foot displacement -v_b*tan(theta/2), shear v_b by
- * +v_a*sin(theta), shear v_a again.  Result: f_out(v) = f_in(R(theta) v).  Exactly one component of B may be
- * non-zero (else BSL6D_EUNSUPPORTED); B == 0 copies f_in to f_out.  One fused pass f_in -> f_out where a fused kernel
- * exists (B along x3 on the specialised extents), else three sweeps: f_in -> f_out, then in place. */
+/* Rotation of velocity space by the background field, dV/dt = V x B (eq (3)), as velocity shears
+ * (BASELINE.json configs[3], reading S7).  B: HOST, 3 doubles, = (q/m)*B0.  Result: f_out(v) = f_in(R(B*dt) v).
+ *   B along one coordinate axis c, (a,b,c) cyclic, theta = B[c]*dt: shear v_a by foot displacement -v_b*tan(theta/2),
+ *     shear v_b by +v_a*sin(theta), shear v_a again -- three sweeps, ONE fused pass f_in -> f_out where a fused kernel
+ *     exists (B along x3 on the specialised extents), else f_in -> f_out and two sweeps in place.
+ *   B in general position (reading R1): with B/|B| = (sin vt cos ph, sin vt sin ph, cos vt) and
+ *     theta = |B|*dt, R = Rz(ph) Ry(vt) Rz(theta) Ry(-vt) Rz(-ph), the five factors applied left to right, each as
+ *     three shears (a factor above pi/2 in equal pieces): 15 or more sweeps, the Rz factors fused.  |theta| <= 2 pi,
+ *     else BSL6D_EUNSUPPORTED.
+ *   B == 0 copies f_in to f_out. */
 BSL6D_API int bsl6d_rotate(bsl6d_ctx* ctx, const double* f_in, double* f_out, const double B[3], double dt, void* stream);
 
 /* One Strang-split time step (order per BASELINE.json configs[4], reading S8), result in f:

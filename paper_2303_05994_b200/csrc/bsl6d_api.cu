@@ -502,23 +502,53 @@ int run_sequence_pingpong(bsl6d_ctx* c, double* f, double* f_tmp, const SweepDes
 
 struct Shear { int dim; int src_dim; double scale; };
 
-// Three shears of the rotation (see bsl6d_rotate in the header).  Returns the number of sweeps (0 or 3).
-int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear out[3], int* count) {
-    *count = 0;
-    if (!std::isfinite(dt)) return BSL6D_EINVAL;
-    int ax = -1;
-    for (int i = 0; i < 3; ++i) {
-        if (!std::isfinite(B[i])) return BSL6D_EINVAL;
-        if (B[i] != 0.0) { if (ax >= 0) return BSL6D_EUNSUPPORTED; ax = i; }
-    }
-    if (ax < 0) return BSL6D_OK;
+constexpr int kMaxShears = 48;                               // 16 axis rotations x 3 shears
+
+// Three shears of a rotation about coordinate axis `ax` by `theta` (see bsl6d_rotate in the header).
+void axis_shears(const bsl6d_ctx* c, int ax, double theta, Shear* out) {
     const int a = (ax + 1) % 3, b = (ax + 2) % 3;
-    const double theta = B[ax] * dt;
     const double t = std::tan(0.5 * theta), s = std::sin(theta);
     out[0] = Shear{3 + a, 3 + b, t / c->g.dx[3 + a]};       // foot displacement -v_b tan(theta/2)
     out[1] = Shear{3 + b, 3 + a, -s / c->g.dx[3 + b]};      // foot displacement +v_a sin(theta)
     out[2] = out[0];
-    *count = 3;
+}
+
+// The shear sequence of the rotation by B*dt.  B along one coordinate axis: three shears.  B in general position
+// (reading R1): with B/|B| = (sin vt cos ph, sin vt sin ph, cos vt) and theta = |B| dt,
+// R(b, theta) = Rz(ph) Ry(vt) Rz(theta) Ry(-vt) Rz(-ph); the factors are applied left to right, each as three shears,
+// a factor above pi/2 in ceil(|angle| / (pi/2)) equal pieces.  |theta| <= 2 pi.  `out` holds kMaxShears entries.
+int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear* out, int* count) {
+    *count = 0;
+    if (!std::isfinite(dt)) return BSL6D_EINVAL;
+    int ax = -1, nz = 0;
+    for (int i = 0; i < 3; ++i) {
+        if (!std::isfinite(B[i])) return BSL6D_EINVAL;
+        if (B[i] != 0.0) { ax = i; ++nz; }
+    }
+    if (nz == 0) return BSL6D_OK;
+    if (nz == 1) {
+        axis_shears(c, ax, B[ax] * dt, out);
+        *count = 3;
+        return BSL6D_OK;
+    }
+    const double bn = std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
+    const double theta = bn * dt;
+    if (std::fabs(theta) > 6.283185307179586477) return BSL6D_EUNSUPPORTED;
+    const double vt = std::acos(B[2] / bn);
+    const double ph = std::atan2(B[1], B[0]);
+    const int axes[5] = {2, 1, 2, 1, 2};
+    const double ang[5] = {ph, vt, theta, -vt, -ph};
+    const double half_pi = 1.5707963267948966;
+    int n = 0;
+    for (int i = 0; i < 5; ++i) {
+        if (ang[i] == 0.0) continue;
+        const int pieces = (int)std::ceil(std::fabs(ang[i]) / half_pi);
+        for (int k = 0; k < pieces && n + 3 <= kMaxShears; ++k) {
+            axis_shears(c, axes[i], ang[i] / (double)pieces, out + n);
+            n += 3;
+        }
+    }
+    *count = n;
     return BSL6D_OK;
 }
 
@@ -700,11 +730,11 @@ int bsl6d_advect(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
 
 int bsl6d_rotate(bsl6d_ctx* c, const double* f_in, double* f_out, const double B[3], double dt, void* stream) {
     if (!c || !f_in || !f_out || !B) return BSL6D_EINVAL;
-    Shear sh[3];
+    Shear sh[kMaxShears];
     int cnt = 0;
     int rc = plan_rotation(c, B, dt, sh, &cnt);
     if (rc) return rc;
-    SweepDesc sw[3];
+    SweepDesc sw[kMaxShears];
     for (int i = 0; i < cnt; ++i)
         sw[i] = SweepDesc{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
     return run_sequence_in_out(c, f_in, f_out, sw, cnt, (cudaStream_t)stream);
@@ -713,7 +743,7 @@ int bsl6d_rotate(bsl6d_ctx* c, const double* f_in, double* f_out, const double B
 int bsl6d_strang_step(bsl6d_ctx* c, double* f, double* f_tmp, const double* const E[3], const double B[3], double dt,
                       void* stream) {
     if (!c || !f || !std::isfinite(dt)) return BSL6D_EINVAL;
-    SweepDesc steps[12];
+    SweepDesc steps[9 + kMaxShears];
     int ns = 0;
     const double half = 0.5 * dt;
     for (int d = 0; d < 3; ++d)
@@ -722,7 +752,7 @@ int bsl6d_strang_step(bsl6d_ctx* c, double* f, double* f_tmp, const double* cons
         for (int d = 0; d < 3; ++d)
             if (E[d]) steps[ns++] = SweepDesc{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
     if (B) {
-        Shear sh[3];
+        Shear sh[kMaxShears];
         int cnt = 0;
         int rc = plan_rotation(c, B, dt, sh, &cnt);
         if (rc) return rc;
@@ -828,7 +858,7 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
     if (!c || !f || !rho || !E || !E[0] || !E[1] || !E[2] || !std::isfinite(dt)) return BSL6D_EINVAL;
     if (closure != 0 && closure != 1) return BSL6D_EINVAL;
     if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
-    Shear sh[3];
+    Shear sh[kMaxShears];
     int cnt = 0;
     if (B) {
         int rc = plan_rotation(c, B, dt, sh, &cnt);
@@ -838,7 +868,7 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const double half = 0.5 * dt;
-    SweepDesc xs[3], vs[9];
+    SweepDesc xs[3], vs[6 + kMaxShears];
     for (int d = 0; d < 3; ++d) xs[d] = SweepDesc{d, c->d_nodes + c->node_off[d + 3], 1u << (d + 3), half / c->g.dx[d]};
     int nv = 0;
     for (int d = 0; d < 3; ++d) vs[nv++] = SweepDesc{3 + d, E[d], 0x7u, dt / c->g.dx[3 + d]};
@@ -894,7 +924,7 @@ int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, co
             if (op.dim >= 3 && !op.shift_source) return BSL6D_EINVAL;
             if (op.shift_source) small += op.dim < 3 ? (size_t)g.n[op.dim + 3] : nx;
         } else if (op.kind == 1) {
-            Shear sh[3];
+            Shear sh[kMaxShears];
             int cnt;
             int rc = plan_rotation(c, op.B, op.dt, sh, &cnt);
             if (rc) return rc;

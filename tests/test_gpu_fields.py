@@ -138,7 +138,7 @@ def test_field_error_paths():
             ctx.field_poisson(rho, float("nan"), 1.0, E)
         assert e.value.code == bsl.EINVAL
         with pytest.raises(bsl.Bsl6dError) as e:
-            ctx.vp_step(f, None, rho, E, (0.1, 0.2, 0.0), 0.1, 0, 1.0, 1.0)      # oblique B
+            ctx.vp_step(f, None, rho, E, (30.0, 40.0, 0.0), 0.2, 0, 1.0, 1.0)    # oblique B, > a full turn
         assert e.value.code == bsl.EUNSUPPORTED
         with pytest.raises(bsl.Bsl6dError) as e:
             ctx.vp_step(f, None, rho, E, None, 0.1, 7, 1.0, 1.0)                 # unknown closure

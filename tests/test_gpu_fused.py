@@ -178,3 +178,26 @@ def test_sequence_error_paths_enqueue_nothing():
         assert ctx.launch_count() == 0
         out = ctx.advect_seq(fd, torch.empty_like(fd), [])   # empty chain copies
         assert torch.equal(out, fd)
+
+
+@pytest.mark.parametrize("B,dt", [((0.4, -0.3, 0.6), 0.5), ((1.0, 1.0, 0.0), 0.4), ((0.0, 1.0, 1.0), 2.5),
+                                  ((-2.0, 0.1, -1.0), 0.9)])
+def test_oblique_B_rotation_matches_oracle(B, dt):
+    """SURVEY.md 8(f) N4: B in general position = five axis rotations of three shears each (same plan as the oracle);
+    the Rz factors run as fused passes.  GPU == oracle within 1e-12, fused == unfused bit for bit."""
+    _need_gpu()
+    w = wl.C4.reduced((2, 1, 2, 16, 16, 16))
+    f = w.make_f("cpu").numpy()
+    fd = torch.from_numpy(f).cuda()
+    nrot = len(oracle.rotation_plan(B, dt))
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        fused = ctx.rotate(fd, torch.empty_like(fd), B, dt)
+        nfused = ctx.launch_count()
+        ctx.set_fusion(0)
+        plain = ctx.rotate(fd, torch.empty_like(fd), B, dt)
+        assert ctx.launch_count() - nfused == 3 * nrot
+        assert nfused < 3 * nrot
+        inplace = fd.clone()
+        ctx.rotate(inplace, inplace, B, dt)
+    assert torch.equal(fused, plain) and torch.equal(inplace, plain)
+    assert rel_err(fused, oracle.rotate(ogrid(w), w.degree, f, B, dt)) <= TOL

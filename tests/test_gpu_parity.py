@@ -363,6 +363,6 @@ def test_error_codes():
             ctx.advect(a, a, 0, None, float("nan"))
         assert e.value.code == bsl.EINVAL
         with pytest.raises(bsl.Bsl6dError) as e:
-            ctx.rotate(a, a, [0.1, 0.2, 0.0], 0.1)            # oblique B
+            ctx.rotate(a, a, [30.0, 40.0, 0.0], 0.2)          # oblique B, more than a full turn
         assert e.value.code == bsl.EUNSUPPORTED
         assert ctx.launch_count() == 0                        # failed calls enqueue nothing
