@@ -19,6 +19,14 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+// Cache hints of the streaming accesses to f (every element is touched once per sweep): evict-first loads and stores.
+#ifndef BSL6D_LD
+#define BSL6D_LD __ldcs
+#endif
+#ifndef BSL6D_ST
+#define BSL6D_ST __stcs
+#endif
+
 namespace bsl6d {
 
 constexpr int kMaxSrcTerms = 5;
@@ -134,7 +142,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
         for (int t = 0; t < N; ++t) {
             int row = r0 + t;
             if (row >= N) row -= N;
-            u[t] = __ldcs(pin + (size_t)row * stride);
+            u[t] = BSL6D_LD(pin + (size_t)row * stride);
         }
     } else {
         // rows r0 .. r0+N+Q-2; anything outside [0,N) is the zero extension
@@ -144,7 +152,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
 #pragma unroll
         for (int t = 0; t < NU; ++t) {
             const int row = r0 + t;
-            u[t] = (row >= 0 && row < N) ? __ldcs(pin + (size_t)row * stride) : 0.0;
+            u[t] = (row >= 0 && row < N) ? BSL6D_LD(pin + (size_t)row * stride) : 0.0;
         }
     }
 
@@ -156,7 +164,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
         double acc = w[0] * u[PERIODIC ? (j % N) : j];
 #pragma unroll
         for (int m = 1; m < Q; ++m) acc = fma(w[m], u[PERIODIC ? ((j + m) % N) : (j + m)], acc);
-        __stcs(pout + (size_t)j * stride, acc);
+        BSL6D_ST(pout + (size_t)j * stride, acc);
     }
 }
 
