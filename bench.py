@@ -454,7 +454,10 @@ def run_ours(args, w):
             "config": {"workload": f"{w.name} (BASELINE configs[1]) fp64 {'x'.join(map(str, w.n))}, degree "
                                    f"{w.degree}: sweeps x1,x2,x3,v1,v2,v3 (dt={w.dt}) + rotation shears v1,v2,v1 "
                                    f"(theta={ROT_DT}) + density, per replica",
-                       "l2": "inputs (8.6 GB per buffer) larger than the 126 MB L2; no flush",
+                       "l2": (f"inputs ({8 * npts / 1e9:.1f} GB per buffer) larger than the 126 MB L2; no flush"
+                              if 8 * npts > 2 * 126e6 else
+                              f"inputs ({8 * npts / 1e6:.1f} MB per buffer) fit in the 126 MB L2: launch-latency-bound, "
+                              "NOT an HBM measurement"),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "wall_ms_per_step": 1e3 * t_wall / K},
             "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
