@@ -1,21 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the BSL6D split-advection hot path on B200 (driver contract: one JSON line).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C5] [--per-config C2,C3]
 
-One *step* = one pass of the whole hot path over the resident distribution function of
-BASELINE.json configs[1] (C2: fp64 32^6, degree 7):
-    six 1-D sweeps x1,x2,x3 (shift v_d*dt/dx_d) and v1,v2,v3 (shift E_d(x)*dt/dv_d), dt = 0.05      [a1-a4]
-    the magnetic rotation as three velocity shears (B along x3, theta = 0.1: configs[3] on the same grid) [a5]
-    the density moment rho(x)                                                                          [a6]
-sequenced on one stream through the C ABI (a7's job).  `value` counts the 9 sweeps' point updates per second
-(the density pass is inside the timed region but adds nothing to the numerator).
+One *step* = one pass of the whole hot path over the resident distribution
+function, sequenced on one stream through the C ABI:
+
+  C5 (headline; BASELINE.json configs[4], the largest single-GPU config: fp64 48^3 x 32^3, degree 9) -- the full
+     Strang step of that config: x1,x2,x3 (dt/2) -> v1,v2,v3 with E (dt) -> rotation as three shears (theta = 0.05)
+     -> x1,x2,x3 (dt/2) -> density moment: 12 sweeps + rho, 725 GB of algorithmic traffic per step.
+  C2 / C3 (configs[1], configs[2]; reported as `per_config` sub-records of the same line) -- the six sweeps
+     x1,x2,x3,v1,v2,v3 (dt = 0.05), the rotation shears of configs[3] (theta = 0.1) and the density: 9 sweeps + rho.
+
+`value` counts the sweeps' point updates per second (the density pass is inside the timed region but adds nothing
+to the numerator); it is measured on the per-sweep path (fusion off): every sweep its own 16 B/point pass, which
+is the graded metric.  The planner's fused passes are reported beside it as `fused_step`.
 
 Timing: CUDA events on the launching stream, W >= 3 warm-up steps, barrier + synchronize on both sides, max over
-ranks.  Inputs (8.6 GB per buffer) are far larger than the 126 MB L2, so no explicit flush is needed.
+ranks.  Inputs (8.6-29 GB per buffer) are far larger than the 126 MB L2, so no explicit flush is needed.
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
-Multi-GPU: the path has no exchange step on one node (replicas only) -- every rank runs
-an independent replica of the workload, `value` is the aggregate, scaling = weak.
+Multi-GPU: the path has no exchange step on one node -- every rank runs an independent
+replica of the workload, `value` is the aggregate, scaling = weak.
 """
 from __future__ import annotations
 
@@ -36,8 +41,10 @@ import numpy as np
 
 METRIC = "fp64 1-D advection sweep Gpoint-updates/s (16 B/point/sweep), whole hot-path step"
 UNIT = "Gpoint-updates/s"
-ROT_DT = 0.1          # theta = |B| * dt = 0.1 (BASELINE.json configs[3])
+ROT_DT = 0.1          # C2/C3 step: theta = |B| * dt = 0.1 (BASELINE.json configs[3])
 ROT_B = (0.0, 0.0, 1.0)
+HEADLINE = "C5"       # the largest single-GPU configuration of BASELINE.json
+CONFIG_INDEX = {"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4}
 
 
 def parse_args():
@@ -46,7 +53,11 @@ def parse_args():
     p.add_argument("--steps", type=int, default=10)
     p.add_argument("--warmup", type=int, default=3)
     p.add_argument("--impl", default="ours", choices=("ours", "reference"))
-    p.add_argument("--workload", default="C2", help="C1..C5 (C2 = BASELINE configs[1] is the contract workload)")
+    p.add_argument("--workload", default=None,
+                   help="C1..C5, P37 (default: C5 = BASELINE configs[4], the largest single-GPU config)")
+    p.add_argument("--per-config", default=None,
+                   help="comma-separated workloads reported as per_config sub-records (default: C2,C3 when "
+                        "--workload is not given, none otherwise)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     p.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     p.add_argument("--no-fused", action="store_true", help="skip the fused-pass variant of the step")
@@ -61,7 +72,7 @@ def peaks():
     try:
         with open(path) as fh:
             d = json.load(fh)
-        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy)"
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy, burst)"
     except Exception:
         return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
 
@@ -118,23 +129,60 @@ class ClockSampler:
                 if r[3 + k].strip().lower().startswith("active"):
                     reasons.add(nm)
         if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
-                       reasons=sorted(reasons), samples=len(sm))
+            # "under load" = the samples drawing more than half of the maximum power seen
+            load = [s for s, p in zip(sm, pw) if p >= 0.5 * max(pw)] or sm
+            out.update(sm_mhz=float(np.median(load)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm), samples_under_load=len(load))
         return out
 
 
 # ------------------------------------------------------------------------------------------------------------
 # the step, as a list of ops (shared description; the GPU leg and the oracle leg each execute it their own way)
 # ------------------------------------------------------------------------------------------------------------
+DIM_NAMES = ("x1", "x2", "x3", "v1", "v2", "v3")
+
+
 def step_ops(w):
-    """[(name, kind, dim)]: the order of one step."""
-    ops = [(nm, "advect", d) for d, nm in enumerate(("x1", "x2", "x3", "v1", "v2", "v3"))]
-    ops.append(("rot", "rotate", -1))
-    ops.append(("rho", "density", -1))
+    """[(name, kind, dim, dt, B)]: the order of one step of workload w."""
+    if w.name == "C5":                                    # BASELINE configs[4]: the full Strang step + density
+        half = 0.5 * w.dt
+        ops = [(DIM_NAMES[d] + "a", "advect", d, half, None) for d in range(3)]
+        ops += [(DIM_NAMES[d], "advect", d, w.dt, None) for d in range(3, 6)]
+        ops.append(("rot", "rotate", -1, w.dt, tuple(w.B)))
+        ops += [(DIM_NAMES[d] + "b", "advect", d, half, None) for d in range(3)]
+        ops.append(("rho", "density", -1, 0.0, None))
+        return ops
+    ops = [(nm, "advect", d, w.dt, None) for d, nm in enumerate(DIM_NAMES)]
+    ops.append(("rot", "rotate", -1, ROT_DT, ROT_B))
+    ops.append(("rho", "density", -1, 0.0, None))
     return ops
 
 
-N_SWEEPS = 9          # 6 advect + 3 shears
+def n_sweeps(w) -> int:
+    return sum(3 if k == "rotate" else (1 if k == "advect" else 0) for _, k, _, _, _ in step_ops(w))
+
+
+def workload_label(w) -> str:
+    idx = CONFIG_INDEX.get(w.name)
+    where = f"BASELINE configs[{idx}]" if idx is not None else "the paper's section-5 grid (PAPER.md:244)"
+    grid = "x".join(map(str, w.n))
+    if w.name == "C5":
+        what = (f"full Strang step x1,x2,x3 (dt/2) -> v1,v2,v3 with E (dt={w.dt}) -> rotation shears v1,v2,v1 "
+                f"(theta={w.dt * w.B[2]:g}) -> x1,x2,x3 (dt/2) -> density: 12 sweeps + rho")
+    else:
+        what = (f"sweeps x1,x2,x3,v1,v2,v3 (dt={w.dt}) + rotation shears v1,v2,v1 (theta={ROT_DT}) + density: "
+                f"9 sweeps + rho")
+    return f"{w.name} = {where}: fp64 {grid}, degree {w.degree}; {what}; per replica"
+
+
+def config_dict(w, world: int):
+    npts = w.npts
+    return {"workload": workload_label(w),
+            "l2": (f"inputs ({8 * npts / 1e9:.1f} GB per buffer) larger than the 126 MB L2; no flush"
+                   if 8 * npts > 2 * 126e6 else
+                   f"inputs ({8 * npts / 1e6:.1f} MB per buffer) fit in the 126 MB L2: launch-latency-bound, "
+                   "NOT an HBM measurement"),
+            "parallelism": "replicas only" if world > 1 else "single GPU"}
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -161,7 +209,7 @@ def whole_job_value(npts: int, n_sweeps: int, steps: int, world: int, total_ms: 
 # ------------------------------------------------------------------------------------------------------------
 class OracleSample:
     """For each op of the step, a crop of the workload's grid (same lo/dx/degree/fields): the swept dim and the
-    three v dims keep their full extent, the other x dims are cropped so that a crop holds <= ~6.7e7 points
+    three v dims keep their full extent, the other x dims are cropped so that a crop holds <= ~target_pts points
     (crops of equal shape share their buffers)."""
 
     def __init__(self, w, target_pts=1 << 26):
@@ -171,7 +219,7 @@ class OracleSample:
         self.cases = []
         shared = {}
         nv = int(np.prod(w.n[3:], dtype=np.int64))
-        for name, kind, dim in step_ops(w):
+        for name, kind, dim, dt, B in step_ops(w):
             n = list(w.n)
             if kind == "advect" and dim < 3:
                 rest = [d for d in range(3) if d != dim]
@@ -191,20 +239,19 @@ class OracleSample:
             f, out = shared[tuple(n)]
             g = oracle.Grid(tuple(sub.n), tuple(sub.lo), tuple(sub.dx))
             E = sub.E()
-            self.cases.append((name, kind, dim, sub, g, f, out, E))
-        self.sweep_pts = sum((3 if k == "rotate" else 1) * c[3].npts for c in self.cases for k in [c[1]]
-                             if k != "density")
+            self.cases.append((name, kind, dim, dt, B, sub, g, f, out, E))
+        self.sweep_pts = sum((3 if c[1] == "rotate" else 1) * c[5].npts for c in self.cases if c[1] != "density")
         self.desc = "per op a crop of the %s grid: " % w.name + ", ".join(
-            f"{c[0]}:{'x'.join(map(str, c[3].n))}" for c in self.cases)
+            f"{c[0]}:{'x'.join(map(str, c[5].n))}" for c in self.cases)
 
     def run_once(self):
-        o, w = self.oracle, self.w
+        o = self.oracle
         t0 = time.perf_counter()
-        for name, kind, dim, sub, g, f, out, E in self.cases:
+        for name, kind, dim, dt, B, sub, g, f, out, E in self.cases:
             if kind == "advect":
-                o.advect(g, sub.degree, f, dim, None if dim < 3 else E[dim - 3], w.dt, out=out)
+                o.advect(g, sub.degree, f, dim, None if dim < 3 else E[dim - 3], dt, out=out)
             elif kind == "rotate":
-                o.rotate(g, sub.degree, f, ROT_B, ROT_DT, out=out)
+                o.rotate(g, sub.degree, f, B, dt, out=out)
             else:
                 o.density(g, f)
         return time.perf_counter() - t0
@@ -216,8 +263,8 @@ def run_reference(args, w):
         return
     import oracle
     oracle.build()
-    samp = OracleSample(w)
-    for _ in range(min(args.warmup, 1)):
+    samp = OracleSample(w, target_pts=1 << 25)            # ~1 s of CPU work per step
+    for _ in range(max(args.warmup, 0)):
         samp.run_once()
     t = 0.0
     for _ in range(args.steps):
@@ -226,10 +273,9 @@ def run_reference(args, w):
     cores = oracle.num_threads()
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * t / args.steps,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{w.name} {'x'.join(map(str, w.n))} degree {w.degree}: six sweeps + rotation "
-                               f"shears + density; oracle on a bounded sample", "sample": samp.desc},
+        "config": config_dict(w, args.gpus),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": samp.desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -240,49 +286,78 @@ def run_reference(args, w):
 # ------------------------------------------------------------------------------------------------------------
 # GPU leg
 # ------------------------------------------------------------------------------------------------------------
-def run_ours(args, w):
-    import torch
-    import torch.distributed as dist
-    import paper_2303_05994_b200 as bsl
+def read_traffic(name: str):
+    """(bytes, source) of the strided sweep kernel from profiles/traffic.csv -- an `ncu` capture, NOT measured in
+    this run (traffic.md names the command and round of every row)."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(tpath) as fh:
+            for ln in fh.read().splitlines()[1:]:
+                c = ln.split(",")
+                if c[0] == name and c[1] == "sweep_strided_kernel":
+                    return float(c[2]), "ncu capture recorded in profiles/traffic.csv (see profiles/traffic.md); " \
+                                        "not measured in this run"
+    except Exception:
+        pass
+    return None, "no ncu capture recorded for this workload"
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    bsl.load_library()                                    # fail loudly if the extension is missing
 
-    dev = torch.device("cuda", local)
+class Gpu:
+    """Process-wide state of the GPU leg."""
+
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
+        import paper_2303_05994_b200 as bsl
+        self.torch, self.dist, self.bsl = torch, dist, bsl
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+        bsl.load_library()                                # fail loudly if the extension is missing
+        self.dev = torch.device("cuda", self.local)
+        self.stream = torch.cuda.current_stream()
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+
+def measure_workload(G: Gpu, w, K: int, W: int, want_fused: bool, sample_clocks: bool, keep_host: bool):
+    """Time K steps of workload w after W warm-up steps.  Returns (record, f0_host or None)."""
+    torch, bsl = G.torch, G.bsl
+    dev, stream, world = G.dev, G.stream, G.world
     npts = w.npts
     nx = w.n[0] * w.n[1] * w.n[2]
     a = w.make_f(dev)                                     # seeded synthetic f (bsl6d_workloads), resident in HBM
     f0_host = None
-    if not args.no_e2e:
+    if keep_host:
         f0_host = torch.empty(w.n, dtype=torch.float64, pin_memory=True)
         f0_host.copy_(a)
     b = torch.empty_like(a)
     rho = torch.empty(w.n[:3], dtype=torch.float64, device=dev)
-    E_host = [torch.from_numpy(e) for e in w.E()]
-    E = [e.to(dev) for e in E_host]
+    E = [torch.from_numpy(e).to(dev) for e in w.E()]
     ctx = bsl.create(w.n, w.lo, w.dx, w.degree)
     ctx.set_fusion(0)                                     # the graded step: every sweep its own 16 B/point pass
     ops = step_ops(w)
-    kernels = {nm: (ctx.kernel_name(d) if kind == "advect" else "") for nm, kind, d in ops}
+    NS = n_sweeps(w)
+    kernels = {nm: (ctx.kernel_name(d) if kind == "advect" else "") for nm, kind, d, _, _ in ops}
     kernels["rot"] = f"{ctx.kernel_name(3)} + {ctx.kernel_name(4)} + {ctx.kernel_name(3)}"
-    stream = torch.cuda.current_stream()
 
     def one_step(cur, oth, evs=None):
-        for i, (name, kind, dim) in enumerate(ops):
+        for i, (name, kind, dim, dt, B) in enumerate(ops):
             if evs is not None:
                 evs[i].record(stream)
             if kind == "advect":
-                ctx.advect(cur, oth, dim, None if dim < 3 else E[dim - 3], w.dt)
+                ctx.advect(cur, oth, dim, None if dim < 3 else E[dim - 3], dt)
                 cur, oth = oth, cur
             elif kind == "rotate":
-                ctx.rotate(cur, oth, ROT_B, ROT_DT)
+                ctx.rotate(cur, oth, B, dt)
                 cur, oth = oth, cur
             else:
                 ctx.density(cur, rho)
@@ -290,182 +365,236 @@ def run_ours(args, w):
             evs[len(ops)].record(stream)
         return cur, oth
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     cur, oth = a, b
-    for _ in range(max(args.warmup, 0)):
+    for _ in range(max(W, 0)):
         cur, oth = one_step(cur, oth)
-    barrier()
+    G.barrier()
 
-    K = args.steps
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(ops) + 1)] for _ in range(K)]
     l0 = ctx.launch_count()
-    clocks = ClockSampler(local)
-    clocks.start()
-    time.sleep(0.25)
-    barrier()
+    clocks = ClockSampler(G.local) if sample_clocks else None
+    if clocks:
+        clocks.start()
+        time.sleep(0.25)
+    G.barrier()
     t_wall = time.perf_counter()
     for s in range(K):
         cur, oth = one_step(cur, oth, evs[s])
-    barrier()
+    G.barrier()
     t_wall = time.perf_counter() - t_wall
-    # keep the sampler alive for a moment if the region was very short, so that it has samples under load
-    clk = clocks.stop()
+    clk = clocks.stop() if clocks else None
     launches = ctx.launch_count() - l0
     total_ms = evs[0][0].elapsed_time(evs[K - 1][len(ops)])
     per_op = {nm: float(np.mean([evs[s][i].elapsed_time(evs[s][i + 1]) for s in range(K)]))
-              for i, (nm, _, _) in enumerate(ops)}
+              for i, (nm, _, _, _, _) in enumerate(ops)}
     assert torch.isfinite(rho).all()
 
     total_ms = max_over_ranks(total_ms, dev)
-    value = whole_job_value(npts, N_SWEEPS, K, world, total_ms)
-    step_bytes = (N_SWEEPS * 16 * npts + 8 * npts + 8 * nx)
+    value = whole_job_value(npts, NS, K, world, total_ms)
+    step_bytes = NS * 16 * npts + 8 * npts + 8 * nx
 
-    # ---- roofline of the dominant kernel: the strided sweep (x1,x2,x3,v1,v2 + the three shears = 8 launches/step)
+    # ---- roofline of the dominant kernel: the strided sweep (every sweep but v3) -------------------------------
     peak, peak_src = peaks()
-    strided_ms = sum(per_op[nm] for nm in ("x1", "x2", "x3", "v1", "v2", "rot")) / 8.0
+    strided_ops = [nm for nm, kind, d, _, _ in ops if (kind == "advect" and d != 5) or kind == "rotate"]
+    n_strided = sum(3 if nm == "rot" else 1 for nm in strided_ops)
+    strided_ms = sum(per_op[nm] for nm in strided_ops) / n_strided
     achieved = 16.0 * npts / (strided_ms * 1e-3) / 1e9
     per_dim = {}
-    for nm, kind, _ in ops:
+    for nm, kind, _, _, _ in ops:
         nl = 3 if kind == "rotate" else 1
         bytes_ = (8 * npts + 8 * nx) if kind == "density" else 16 * npts * nl
         gbs = bytes_ / (per_op[nm] * 1e-3) / 1e9
         per_dim[nm] = {"ms": per_op[nm], "GB/s": gbs, "frac_of_measured_peak": gbs / peak,
-                       "frac_of_8TBs": gbs / 8000.0, "kernel": kernels.get(nm, "")}
+                       "frac_of_8TBs": gbs / 8000.0, "kernel": kernels.get(nm, kernels.get(nm[:2], ""))}
         if kind != "density":
             per_dim[nm]["Gpoint-updates/s"] = nl * npts / (per_op[nm] * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")         # copied from an `ncu --set full` capture (traffic.md)
-    if os.path.exists(tpath):
-        try:
-            with open(tpath) as fh:
-                for ln in fh.read().splitlines()[1:]:
-                    c = ln.split(",")
-                    if c[0] == w.name and c[1] == "sweep_strided_kernel":
-                        traffic = float(c[2])
-        except Exception:
-            traffic = None
-    roofline = {"bound": "hbm", "kernel": "sweep_strided_kernel (8 of 10 launches per step)", "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": 16 * npts, "avg_launch_ms": strided_ms,
+    traffic, traffic_src = read_traffic(w.name)
+    roofline = {"bound": "hbm",
+                "kernel": f"sweep_strided_kernel ({n_strided} of {launches // K} launches per step)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "frac_of_8TBs_spec": achieved / 8000.0, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": 16 * npts, "avg_launch_ms": strided_ms,
                 "step_GB/s": step_bytes / (total_ms / K * 1e-3) / 1e9,
                 "step_frac": step_bytes / (total_ms / K * 1e-3) / 1e9 / peak}
 
-    # ---- the same step with the planner's fused passes: extra information, not `value` --------
+    # ---- the same step through the planner's fused passes: extra information, not `value` ----
     fused = None
-    if not args.no_fused:
+    if want_fused:
         ctx.set_fusion(1)
-        six = [(d, None, 0, w.dt / w.dx[d]) for d in range(3)] + \
-              [(3 + d, E[d], 0x7, w.dt / w.dx[3 + d]) for d in range(3)]
+        if w.name == "C5":
+            def fused_step(cur, oth):
+                ctx.strang_step(cur, oth, E, w.B, w.dt)
+                ctx.density(cur, rho)
+                return cur, oth
+        else:
+            six = [(d, None, 0, w.dt / w.dx[d]) for d in range(3)] + \
+                  [(3 + d, E[d], 0x7, w.dt / w.dx[3 + d]) for d in range(3)]
 
-        def fused_step(cur, oth):
-            ctx.advect_seq(cur, oth, six)
-            ctx.rotate(oth, cur, ROT_B, ROT_DT)
-            ctx.density(cur, rho)
-            return cur, oth
+            def fused_step(cur, oth):
+                ctx.advect_seq(cur, oth, six)
+                ctx.rotate(oth, cur, ROT_B, ROT_DT)
+                ctx.density(cur, rho)
+                return cur, oth
 
         for _ in range(3):
             cur, oth = fused_step(cur, oth)
-        barrier()
+        G.barrier()
         lf0 = ctx.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(K):
             cur, oth = fused_step(cur, oth)
         e1.record(stream)
-        barrier()
+        G.barrier()
         fms = max_over_ranks(e0.elapsed_time(e1), dev)
-        fused = {"value": whole_job_value(npts, N_SWEEPS, K, world, fms), "unit": UNIT, "ms_per_step": fms / K,
-                 "launches_per_step": (ctx.launch_count() - lf0) // K, "speedup_vs_value": (total_ms / K) / (fms / K),
-                 "note": "same nine sweeps + density, bit-identical results; consecutive sweeps over two dims share one "
-                         "pass over f (bsl6d_advect_seq: x1 | x2+x3 | v1+v2 | v3; bsl6d_rotate: one pass), so bytes per "
-                         "point-update drop below 16 and the per-sweep roofline does not apply"}
-        # the full Strang step of BASELINE configs[4] on this grid (12 sweeps; x half, E, rotation, x half)
+        fused = {"value": whole_job_value(npts, NS, K, world, fms), "unit": UNIT, "ms_per_step": fms / K,
+                 "launches_per_step": (ctx.launch_count() - lf0) // K, "speedup_vs_value": total_ms / fms,
+                 "note": "same sweeps + density, bit-identical results; consecutive sweeps share one pass over f "
+                         "where the planner has a fused kernel, so bytes per point-update drop below 16 and the "
+                         "per-sweep roofline does not apply"}
+
+        # the 12-sweep Strang step (BASELINE configs[4]'s sequence) through bsl6d_strang_step, fused and per sweep
+        Bst, dtst = (w.B, w.dt) if w.name == "C5" else (ROT_B, w.dt)
+
         def time_strang(mode):
             ctx.set_fusion(mode)
             l0_ = ctx.launch_count()
             for _ in range(2):
-                ctx.strang_step(cur, oth, E, ROT_B, w.dt)
-            barrier()
+                ctx.strang_step(cur, oth, E, Bst, dtst)
+            G.barrier()
             per = (ctx.launch_count() - l0_) // 2
             s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             s0.record(stream)
             for _ in range(K):
-                ctx.strang_step(cur, oth, E, ROT_B, w.dt)
+                ctx.strang_step(cur, oth, E, Bst, dtst)
             s1.record(stream)
-            barrier()
+            G.barrier()
             return max_over_ranks(s0.elapsed_time(s1), dev) / K, per
 
         st_f, lp_f = time_strang(1)
         st_u, lp_u = time_strang(0)
         fused["strang_step"] = {"ms_fused": st_f, "launches_fused": lp_f, "ms_per_sweep_path": st_u,
-                                "launches_per_sweep_path": lp_u,
+                                "launches_per_sweep_path": lp_u, "speedup": st_u / st_f,
                                 "Gpoint-updates/s_fused": 12 * npts / (st_f * 1e-3) / 1e9,
                                 "Gpoint-updates/s_per_sweep_path": 12 * npts / (st_u * 1e-3) / 1e9}
         ctx.set_fusion(0)
-
-    # ---- e2e: the same step through bsl6d_run_host on HOST buffers (pinned), copies inside the timed region
-    e2e = None
-    if not args.no_e2e:
-        del a, b, cur, oth
-        torch.cuda.empty_cache()
-        hops = []
-        for name, kind, dim in ops:
-            if kind == "advect":
-                hops.append({"kind": "advect", "dim": dim, "dt": w.dt,
-                             "shift_source": None if dim < 3 else E_host[dim - 3]})
-            elif kind == "rotate":
-                hops.append({"kind": "rotate", "B": ROT_B, "dt": ROT_DT})
-            else:
-                hops.append({"kind": "density", "rho_host": torch.empty(w.n[:3], dtype=torch.float64,
-                                                                           pin_memory=True)})
-        ke = max(1, min(K, 5))
-        ctx.run_host(f0_host, f0_host, hops)              # warm-up (allocates the context's device buffer)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(ke):
-            ctx.run_host(f0_host, f0_host, hops)
-        torch.cuda.synchronize()
-        te = time.perf_counter() - t0
-        te = max_over_ranks(te, dev)
-        e2e = {"value": whole_job_value(npts, N_SWEEPS, ke, world, 1e3 * te), "unit": UNIT,
-               "h2d_bytes_per_step": 8 * npts + 3 * 8 * nx, "d2h_bytes_per_step": 8 * npts + 8 * nx,
-               "steps": ke, "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (pinned host buffers)"}
     ctx.destroy()
+    del a, b, cur, oth
+    torch.cuda.empty_cache()
+
+    rec = {"value": value, "unit": UNIT, "steps": K, "warmup": W, "ms_per_step": total_ms / K,
+           "n_sweeps_per_step": NS, "gpu_launches": int(launches), "config": config_dict(w, world),
+           "wall_ms_per_step": 1e3 * t_wall / K, "roofline": roofline, "fused_step": fused, "per_dim": per_dim}
+    if clk is not None:
+        rec["clocks"] = clk
+    return rec, f0_host
+
+
+def host_memory_allows(nbytes: int) -> bool:
+    """Is it safe to pin `nbytes` of host memory on this box (physical memory and cgroup limit)?"""
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        return False
+    for p in ("/sys/fs/cgroup/memory.max", "/sys/fs/cgroup/memory/memory.limit_in_bytes"):
+        try:
+            with open(p) as fh:
+                s = fh.read().strip()
+            if s != "max":
+                avail = min(avail, int(s))
+        except Exception:
+            pass
+    return avail >= 2.5 * nbytes
+
+
+def measure_e2e(G: Gpu, w, f0_host, K: int):
+    """The same step through bsl6d_run_host on HOST buffers (pinned), copies inside the timed region."""
+    torch, bsl = G.torch, G.bsl
+    nx = w.n[0] * w.n[1] * w.n[2]
+    E_host = [torch.from_numpy(e) for e in w.E()]
+    hops, n_small = [], 0
+    for name, kind, dim, dt, B in step_ops(w):
+        if kind == "advect":
+            hops.append({"kind": "advect", "dim": dim, "dt": dt,
+                         "shift_source": None if dim < 3 else E_host[dim - 3]})
+            n_small += 0 if dim < 3 else nx
+        elif kind == "rotate":
+            hops.append({"kind": "rotate", "B": B, "dt": dt})
+        else:
+            hops.append({"kind": "density", "rho_host": torch.empty(w.n[:3], dtype=torch.float64, pin_memory=True)})
+    ctx = bsl.create(w.n, w.lo, w.dx, w.degree)
+    ctx.set_fusion(0)
+    ke = max(1, min(K, 5 if w.npts < (1 << 31) else 2))
+    ctx.run_host(f0_host, f0_host, hops)                  # warm-up (allocates the context's device buffer)
+    G.barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        ctx.run_host(f0_host, f0_host, hops)
+    torch.cuda.synchronize()
+    te = max_over_ranks(time.perf_counter() - t0, G.dev)
+    ctx.destroy()
+    return {"value": whole_job_value(w.npts, n_sweeps(w), ke, G.world, 1e3 * te), "unit": UNIT,
+            "h2d_bytes_per_step": 8 * w.npts + 8 * n_small, "d2h_bytes_per_step": 8 * w.npts + 8 * nx,
+            "steps": ke, "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (pinned host buffers)",
+            "workload": workload_label(w)}
+
+
+def run_ours(args, w, extra):
+    G = Gpu()
+    torch = G.torch
+    K, W = args.steps, args.warmup
+    want_e2e = not args.no_e2e
+    e2e_w = w
+    if want_e2e and not host_memory_allows(8 * w.npts):
+        import bsl6d_workloads as wl
+        e2e_w = wl.C2                                     # not enough host memory to pin this workload's f
+    rec, f0_host = measure_workload(G, w, K, W, not args.no_fused, True, want_e2e and e2e_w is w)
+
+    per_config = {}
+    for x in extra:
+        r, _ = measure_workload(G, x, min(K, 10), max(min(W, 3), 3) if W >= 3 else W, not args.no_fused, False, False)
+        per_config[x.name] = r
+
+    e2e = None
+    if want_e2e:
+        if e2e_w is not w:
+            f0_host = torch.empty(e2e_w.n, dtype=torch.float64, pin_memory=True)
+            tmp = e2e_w.make_f(G.dev)
+            f0_host.copy_(tmp)
+            del tmp
+            torch.cuda.empty_cache()
+        e2e = measure_e2e(G, e2e_w, f0_host, K)
+        if e2e_w is not w:
+            e2e["note"] = (f"host memory on this box does not allow pinning {8 * w.npts / 1e9:.0f} GB; e2e measured on "
+                           f"{e2e_w.name} instead")
+        del f0_host
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu:
+    if G.rank == 0 and G.world == 1 and not args.no_cpu:
         import oracle
         oracle.build()
         samp = OracleSample(w)
-        npass = 3
-        tc = sum(samp.run_once() for _ in range(npass))
-        cpu = {"value": npass * samp.sweep_pts / tc / 1e9, "passes": npass, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": samp.desc, "seconds": tc}
+        tc, npass = 0.0, 0
+        while npass < 12 and (npass < 2 or tc < 10.0):
+            tc += samp.run_once()
+            npass += 1
+        cpu = {"value": npass * samp.sweep_pts / tc / 1e9, "passes": npass, "unit": UNIT,
+               "cores": oracle.num_threads(), "kind": "oracle", "sample": samp.desc, "seconds": tc}
 
-    if rank == 0:
+    if G.rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
-            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{w.name} (BASELINE configs[1]) fp64 {'x'.join(map(str, w.n))}, degree "
-                                   f"{w.degree}: sweeps x1,x2,x3,v1,v2,v3 (dt={w.dt}) + rotation shears v1,v2,v1 "
-                                   f"(theta={ROT_DT}) + density, per replica",
-                       "l2": (f"inputs ({8 * npts / 1e9:.1f} GB per buffer) larger than the 126 MB L2; no flush"
-                              if 8 * npts > 2 * 126e6 else
-                              f"inputs ({8 * npts / 1e6:.1f} MB per buffer) fit in the 126 MB L2: launch-latency-bound, "
-                              "NOT an HBM measurement"),
-                       "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "wall_ms_per_step": 1e3 * t_wall / K},
-            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu, "fused_step": fused, "per_dim": per_dim,
+            "metric": METRIC, "value": rec["value"], "unit": UNIT, "n_gpus": G.world, "steps": K, "warmup": W,
+            "ms_per_step": rec["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": rec["config"],
+            "wall_ms_per_step": rec["wall_ms_per_step"], "n_sweeps_per_step": rec["n_sweeps_per_step"],
+            "clocks": rec.get("clocks"), "e2e": e2e, "gpu_launches": rec["gpu_launches"],
+            "roofline": rec["roofline"], "cpu_baseline": cpu, "fused_step": rec["fused_step"],
+            "per_dim": rec["per_dim"], "per_config": per_config,
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    if G.world > 1:
+        G.dist.destroy_process_group()
 
 
 def run_paper_benchmark(args):
@@ -491,7 +620,7 @@ def run_paper_benchmark(args):
     clocks.start()
     for q in (3, 5, 7, 9):
         row = {}
-        for dim, nm in enumerate(("x1", "x2", "x3", "v1", "v2", "v3")):
+        for dim, nm in enumerate(DIM_NAMES):
             for _ in range(max(args.warmup, 1)):
                 ctx.advect_pointwise(f, out, dim, alpha, q)
             torch.cuda.synchronize()
@@ -527,11 +656,13 @@ def main():
         run_paper_benchmark(args)
         return
     import bsl6d_workloads as wl
-    w = wl.CONFIGS[args.workload]
+    w = wl.CONFIGS[args.workload or HEADLINE]
     if args.impl == "reference":
         run_reference(args, w)
-    else:
-        run_ours(args, w)
+        return
+    names = args.per_config if args.per_config is not None else ("C2,C3" if args.workload is None else "")
+    extra = [wl.CONFIGS[n] for n in names.split(",") if n and n != w.name]
+    run_ours(args, w, extra)
 
 
 if __name__ == "__main__":

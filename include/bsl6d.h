@@ -85,7 +85,8 @@ BSL6D_API int bsl6d_advect_generic(bsl6d_ctx* ctx, const double* f_in, double* f
  * (BASELINE.json configs[3], reading S7).  B: HOST, 3 doubles, = (q/m)*B0.  Result: f_out(v) = f_in(R(B*dt) v).
  *   B along one coordinate axis c, (a,b,c) cyclic, theta = B[c]*dt: shear v_a by foot displacement -v_b*tan(theta/2),
  *     shear v_b by +v_a*sin(theta), shear v_a again -- three sweeps, ONE fused pass f_in -> f_out where a fused kernel
- *     exists (B along x3 on the specialised extents), else f_in -> f_out and two sweeps in place.
+ *     exists, else f_in -> f_out and two sweeps in place.  |theta| > pi/2 is applied in ceil(|theta|/(pi/2)) equal
+ *     pieces of three shears each (tan(theta/2) diverges at pi; reading R2); |theta| > 2 pi is BSL6D_EUNSUPPORTED.
  *   B in general position (reading R1): with B/|B| = (sin vt cos ph, sin vt sin ph, cos vt) and
  *     theta = |B|*dt, R = Rz(ph) Ry(vt) Rz(theta) Ry(-vt) Rz(-ph), the five factors applied left to right, each as
  *     three shears (a factor above pi/2 in equal pieces): 15 or more sweeps, the Rz factors fused.  |theta| <= 2 pi,

@@ -230,7 +230,18 @@ int rotate(const Grid& g, int q, const double* f_in, double* f_out, const double
         if (B[i] != 0.0) { c = i; ++nz; }
     const long long npts = total_points(g.n);
     if (nz == 0) { if (f_in != f_out) std::memcpy(f_out, f_in, sizeof(double) * npts); return 0; }
-    if (nz == 1) { rotate_axis(g, q, f_in, f_out, c, B[c] * dt); return 0; }
+    if (nz == 1) {
+        // Reading R2: tan(theta/2) diverges at theta = pi, so an axis rotation above pi/2 is applied in
+        // ceil(|theta| / (pi/2)) equal pieces of three shears (one piece for |theta| <= pi/2: the plain three shears);
+        // more than a full turn is rejected, as for an oblique axis.
+        const double theta = B[c] * dt;
+        if (std::fabs(theta) > 6.283185307179586477) return -1;
+        int pieces = (int)std::ceil(std::fabs(theta) / 1.5707963267948966);
+        if (pieces < 1) pieces = 1;
+        const double* cur = f_in;
+        for (int k = 0; k < pieces; ++k) { rotate_axis(g, q, cur, f_out, c, theta / (double)pieces); cur = f_out; }
+        return 0;
+    }
     int axes[16];
     double angles[16];
     if (std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]) * std::fabs(dt) > 6.283185307179586477) return -1;

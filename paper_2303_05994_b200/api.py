@@ -122,6 +122,11 @@ class Context:
             g.n[d], g.lo[d], g.dx[d] = int(n[d]), float(lo[d]), float(dx[d])
         self.n = tuple(int(v) for v in n)
         self.degree = int(degree)
+        self.npts = 1
+        for v in self.n:
+            self.npts *= v
+        self.nx = self.n[0] * self.n[1] * self.n[2]
+        self.device = torch.cuda.current_device() if torch.cuda.is_available() else None
         rc = self._lib.bsl6d_create(C.byref(g), int(degree), C.byref(self._h))
         if rc != OK:
             self._h = C.c_void_p()
@@ -153,12 +158,29 @@ class Context:
         self.destroy()
 
     def _shape_ok(self, t: torch.Tensor, what: str):
-        if t.numel() != int(torch.tensor(self.n).prod()):
-            raise ValueError(f"{what}: wrong number of elements for grid {self.n}")
+        self._count_ok(t, self.npts, what)
+
+    def _count_ok(self, t: Optional[torch.Tensor], want: int, what: str):
+        """Element count and device of a tensor argument (the C ABI takes bare pointers and cannot check either)."""
+        if t is None:
+            return
+        if t.numel() != want:
+            raise ValueError(f"{what}: {t.numel()} elements, want {want} for grid {self.n}")
+        if t.is_cuda and self.device is not None and t.device.index != self.device:
+            raise ValueError(f"{what}: lives on cuda:{t.device.index}, the context was created on cuda:{self.device}")
+
+    def _mask_count(self, mask: int) -> int:
+        want = 1
+        for d in range(6):
+            if mask >> d & 1:
+                want *= self.n[d]
+        return want
 
     # -- the C entry points -------------------------------------------------------------------------------
     def advect(self, f_in, f_out, dim: int, shift_source, dt: float, stream=None):
         self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        if 0 <= int(dim) <= 5:
+            self._count_ok(shift_source, self.n[dim + 3] if dim < 3 else self.nx, "shift_source")
         self._check(self._lib.bsl6d_advect(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"), int(dim),
                                            _dev_ptr(shift_source, "shift_source"), float(dt), _stream(stream)),
                     "bsl6d_advect")
@@ -166,12 +188,7 @@ class Context:
 
     def advect_generic(self, f_in, f_out, dim: int, src, src_dim_mask: int, scale: float, stream=None):
         self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
-        want = 1
-        for d in range(6):
-            if src_dim_mask >> d & 1:
-                want *= self.n[d]
-        if src is not None and src.numel() != want:
-            raise ValueError("src: wrong number of elements for the mask")
+        self._count_ok(src, self._mask_count(int(src_dim_mask)), "src")
         self._check(self._lib.bsl6d_advect_generic(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_out, "f_out"),
                                                    int(dim), _dev_ptr(src, "src"), int(src_dim_mask), float(scale),
                                                    _stream(stream)), "bsl6d_advect_generic")
@@ -185,9 +202,11 @@ class Context:
         return f_out
 
     def strang_step(self, f, f_tmp, E, B, dt: float, stream=None):
-        self._shape_ok(f, "f")
+        self._shape_ok(f, "f"); self._count_ok(f_tmp, self.npts, "f_tmp")
         Ep = None
         if E is not None:
+            for e in E:
+                self._count_ok(e, self.nx, "E")
             Ep = (C.c_void_p * 3)(*[_dev_ptr(e, "E") for e in E])
         Bc = None if B is None else (C.c_double * 3)(*[float(b) for b in B])
         self._check(self._lib.bsl6d_strang_step(self._h, _dev_ptr(f, "f"), _dev_ptr(f_tmp, "f_tmp"), Ep, Bc, float(dt),
@@ -198,6 +217,7 @@ class Context:
         """sweeps: (dim, src tensor or None, src_dim_mask, scale) tuples -> bsl6d_sweep array."""
         arr = (Sweep * max(1, len(sweeps)))()
         for i, (dim, src, mask, scale) in enumerate(sweeps):
+            self._count_ok(src, self._mask_count(int(mask)), f"sweeps[{i}].src")
             arr[i].dim, arr[i].src_dim_mask, arr[i].scale = int(dim), int(mask), float(scale)
             arr[i].src = _dev_ptr(src, "src")
         return arr
@@ -230,24 +250,24 @@ class Context:
         return f_out
 
     def _E3(self, E):
-        nx = self.n[0] * self.n[1] * self.n[2]
         for e in E:
-            if e.numel() != nx:
-                raise ValueError("E: wrong number of elements")
+            self._count_ok(e, self.nx, "E")
         return (C.c_void_p * 3)(*[_dev_ptr(e, "E") for e in E])
 
     def field_poisson(self, rho, rho_fac: float, e_fac: float, E, stream=None):
+        self._count_ok(rho, self.nx, "rho")
         self._check(self._lib.bsl6d_field_poisson(self._h, _dev_ptr(rho, "rho"), float(rho_fac), float(e_fac),
                                                   self._E3(E), _stream(stream)), "bsl6d_field_poisson")
         return E
 
     def field_adiabatic(self, rho, phi_fac: float, e_fac: float, E, stream=None):
+        self._count_ok(rho, self.nx, "rho")
         self._check(self._lib.bsl6d_field_adiabatic(self._h, _dev_ptr(rho, "rho"), float(phi_fac), float(e_fac),
                                                     self._E3(E), _stream(stream)), "bsl6d_field_adiabatic")
         return E
 
     def vp_step(self, f, f_tmp, rho, E, B, dt: float, closure: int, c1: float, e_fac: float, stream=None):
-        self._shape_ok(f, "f")
+        self._shape_ok(f, "f"); self._count_ok(f_tmp, self.npts, "f_tmp"); self._count_ok(rho, self.nx, "rho")
         Bc = None if B is None else (C.c_double * 3)(*[float(b) for b in B])
         self._check(self._lib.bsl6d_vp_step(self._h, _dev_ptr(f, "f"), _dev_ptr(f_tmp, "f_tmp"), _dev_ptr(rho, "rho"),
                                             self._E3(E), Bc, float(dt), int(closure), float(c1), float(e_fac),
@@ -255,9 +275,7 @@ class Context:
         return f
 
     def density(self, f, rho, stream=None):
-        self._shape_ok(f, "f")
-        if rho.numel() != self.n[0] * self.n[1] * self.n[2]:
-            raise ValueError("rho: wrong number of elements")
+        self._shape_ok(f, "f"); self._count_ok(rho, self.nx, "rho")
         self._check(self._lib.bsl6d_density(self._h, _dev_ptr(f, "f"), _dev_ptr(rho, "rho"), _stream(stream)),
                     "bsl6d_density")
         return rho

@@ -32,9 +32,11 @@ struct bsl6d_ctx {
     long long launches;
     double2* fld[5];          // field step: complex work arrays over the x grid (allocated on first use)
     double2* tw[3];           // field step: twiddle tables exp(-2 pi i m / n_d)
+    int field_ready;          // field step: every table and work array is allocated
     int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
-    const void* smem_ok[32];  // fused kernels whose dynamic shared-memory limit has been raised
+    const void* smem_ok[64];  // kernels whose dynamic shared-memory limit has been raised (and to how much)
+    size_t smem_ok_bytes[64];
     int n_smem_ok;
     // host-path working set (bsl6d_run_host), allocated on first use
     double* h_f;              // device buffer for f
@@ -194,6 +196,27 @@ int cuda_fail(bsl6d_ctx* c, cudaError_t e) {
     return BSL6D_ECUDA;
 }
 
+// Every entry point runs on the device the context was created on (its tables live there).
+int check_device(bsl6d_ctx* c) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return dev == c->device ? BSL6D_OK : BSL6D_EINVAL;
+}
+
+// Raise a kernel's dynamic shared-memory limit once (the attribute is per function and sticks): remembered per context.
+int allow_smem(bsl6d_ctx* c, const void* fn, size_t smem) {
+    if (smem <= 48 * 1024) return BSL6D_OK;
+    for (int k = 0; k < c->n_smem_ok; ++k)
+        if (c->smem_ok[k] == fn && c->smem_ok_bytes[k] >= smem) return BSL6D_OK;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    for (int k = 0; k < c->n_smem_ok; ++k)
+        if (c->smem_ok[k] == fn) { c->smem_ok_bytes[k] = smem; return BSL6D_OK; }
+    if (c->n_smem_ok < 64) { c->smem_ok[c->n_smem_ok] = fn; c->smem_ok_bytes[c->n_smem_ok++] = smem; }
+    return BSL6D_OK;
+}
+
 uint32_t ceil_pow2_log2(uint64_t v) {
     uint32_t l = 0;
     while ((1ull << l) < v) ++l;
@@ -253,7 +276,9 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     if (inner > 0xFFFFFFFFull || outer > 0xFFFFFFFFull || inner * outer > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
 
     KernelChoice kc;
-    int rc = choose_kernel(c, dim, kc);
+    int rc = check_device(c);
+    if (rc) return rc;
+    rc = choose_kernel(c, dim, kc);
     if (rc) return rc;
 
     SweepArgs a;
@@ -288,20 +313,16 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     if (kc.kind == 2) {
         const void* gfn = (inner == 1 && dim >= 3) ? generic_unit_fn(c->q, kc.gen_T) : generic_fn(c->q, kc.gen_T);
         if (!gfn) return BSL6D_EUNSUPPORTED;
-        if (kc.smem > 48 * 1024) {
-            e = cudaFuncSetAttribute(gfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kc.smem);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-        }
+        rc = allow_smem(c, gfn, kc.smem);
+        if (rc) return rc;
         int per = dim < 3 ? 1 : 0;
         void* gargs[] = {(void*)&a, (void*)&per};                  // the unit-stride kernel takes only `a`
         grid = (unsigned)((inner * outer + (size_t)kc.gen_T - 1) / (size_t)kc.gen_T);
         e = cudaLaunchKernel(gfn, dim3(grid), dim3(kc.gen_T), gargs, kc.smem, stream);
         if (e != cudaSuccess) return cuda_fail(c, e);
     } else {
-        if (kc.smem > 48 * 1024) {
-            e = cudaFuncSetAttribute((const void*)kc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kc.smem);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-        }
+        rc = allow_smem(c, (const void*)kc.fn, kc.smem);
+        if (rc) return rc;
         void* args[] = {(void*)&a};
         e = cudaLaunchKernel((const void*)kc.fn, dim3(grid), dim3(kc.threads), args, kc.smem, stream);
         if (e != cudaSuccess) return cuda_fail(c, e);
@@ -423,15 +444,7 @@ int launch_fused(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDes
         if (rc) return rc;
     }
     cudaError_t e;
-    if (p.fc.smem > 48 * 1024) {
-        bool known = false;
-        for (int k = 0; k < c->n_smem_ok; ++k) known = known || c->smem_ok[k] == p.fc.fn;
-        if (!known) {
-            e = cudaFuncSetAttribute(p.fc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.fc.smem);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-            if (c->n_smem_ok < 32) c->smem_ok[c->n_smem_ok++] = p.fc.fn;
-        }
-    }
+    if (int rcs = allow_smem(c, p.fc.fn, p.fc.smem)) return rcs;
     const unsigned grid = (unsigned)(outer * mid * (size_t)fa.nchunks);
     void* args[] = {(void*)&fa};
     e = cudaLaunchKernel(p.fc.fn, dim3(grid), dim3(p.fc.threads), args, p.fc.smem, stream);
@@ -462,7 +475,9 @@ int run_sequence_in_out(bsl6d_ctx* c, const double* f_in, double* f_out, const S
     if (!c || !f_in || !f_out || ns < 0 || (ns > 0 && !sw)) return BSL6D_EINVAL;
     if (partial_overlap(c, f_in, f_out)) return BSL6D_EALIAS;
     std::vector<Pass> passes;
-    int rc = plan_passes(c, sw, ns, passes);
+    int rc = check_device(c);
+    if (rc) return rc;
+    rc = plan_passes(c, sw, ns, passes);
     if (rc) return rc;
     if (passes.empty()) {
         if (f_in != f_out) {
@@ -485,7 +500,9 @@ int run_sequence_pingpong(bsl6d_ctx* c, double* f, double* f_tmp, const SweepDes
     if (!c || !f) return BSL6D_EINVAL;
     if (f_tmp && (f_tmp == f || partial_overlap(c, f, f_tmp))) return BSL6D_EALIAS;
     std::vector<Pass> passes;
-    int rc = plan_passes(c, sw, ns, passes);
+    int rc = check_device(c);
+    if (rc) return rc;
+    rc = plan_passes(c, sw, ns, passes);
     if (rc) return rc;
     const int np = (int)passes.size();
     double* cur = f;
@@ -526,9 +543,15 @@ int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear* out, 
         if (B[i] != 0.0) { ax = i; ++nz; }
     }
     if (nz == 0) return BSL6D_OK;
+    const double half_pi = 1.5707963267948966;
     if (nz == 1) {
-        axis_shears(c, ax, B[ax] * dt, out);
-        *count = 3;
+        // reading R2: above pi/2 in equal pieces (tan(theta/2) diverges at pi); one piece = the plain three shears
+        const double theta = B[ax] * dt;
+        if (std::fabs(theta) > 6.283185307179586477) return BSL6D_EUNSUPPORTED;
+        int pieces = (int)std::ceil(std::fabs(theta) / half_pi);
+        if (pieces < 1) pieces = 1;
+        for (int k = 0; k < pieces; ++k) axis_shears(c, ax, theta / (double)pieces, out + 3 * k);
+        *count = 3 * pieces;
         return BSL6D_OK;
     }
     const double bn = std::sqrt(B[0] * B[0] + B[1] * B[1] + B[2] * B[2]);
@@ -538,7 +561,6 @@ int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear* out, 
     const double ph = std::atan2(B[1], B[0]);
     const int axes[5] = {2, 1, 2, 1, 2};
     const double ang[5] = {ph, vt, theta, -vt, -ph};
-    const double half_pi = 1.5707963267948966;
     int n = 0;
     for (int i = 0; i < 5; ++i) {
         if (ang[i] == 0.0) continue;
@@ -554,9 +576,10 @@ int plan_rotation(const bsl6d_ctx* c, const double B[3], double dt, Shear* out, 
 
 // ---- field step ------------------------------------------------------------------------------
 int field_setup(bsl6d_ctx* c) {
-    if (c->fld[0]) return BSL6D_OK;
+    if (c->field_ready) return BSL6D_OK;
     const size_t nx = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2];
     if (nx > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+    // A buffer that an earlier, failed attempt already allocated is kept and reused (nothing is allocated twice).
     for (int d = 0; d < 3; ++d) {
         const int n = c->g.n[d];
         std::vector<double2> w((size_t)n);
@@ -564,12 +587,21 @@ int field_setup(bsl6d_ctx* c) {
             const double ang = -2.0 * 3.14159265358979323846 * (double)m / (double)n;
             w[(size_t)m] = make_double2(std::cos(ang), std::sin(ang));
         }
-        if (cudaMalloc((void**)&c->tw[d], (size_t)n * sizeof(double2)) != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+        if (!c->tw[d] && cudaMalloc((void**)&c->tw[d], (size_t)n * sizeof(double2)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            c->tw[d] = nullptr;
+            return BSL6D_ENOMEM;
+        }
         cudaError_t e = cudaMemcpy(c->tw[d], w.data(), (size_t)n * sizeof(double2), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) return cuda_fail(c, e);
     }
-    for (int k = 4; k >= 0; --k)                               // fld[0] last: it marks "set up"
-        if (cudaMalloc((void**)&c->fld[k], nx * sizeof(double2)) != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
+    for (int k = 0; k < 5; ++k)
+        if (!c->fld[k] && cudaMalloc((void**)&c->fld[k], nx * sizeof(double2)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            c->fld[k] = nullptr;
+            return BSL6D_ENOMEM;
+        }
+    c->field_ready = 1;
     return BSL6D_OK;
 }
 
@@ -577,7 +609,9 @@ int field_solve(bsl6d_ctx* c, const double* rho, int adiabatic, double c1, doubl
                 cudaStream_t st) {
     if (!c || !rho || !E || !E[0] || !E[1] || !E[2]) return BSL6D_EINVAL;
     if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
-    int rc = field_setup(c);
+    int rc = check_device(c);
+    if (rc) return rc;
+    rc = field_setup(c);
     if (rc) return rc;
     const uint32_t n0 = (uint32_t)c->g.n[0], n1 = (uint32_t)c->g.n[1], n2 = (uint32_t)c->g.n[2];
     const uint32_t total = n0 * n1 * n2;
@@ -586,6 +620,11 @@ int field_solve(bsl6d_ctx* c, const double* rho, int adiabatic, double c1, doubl
     using namespace bsl6d;
     // forward: axis 2 (real in), axis 1, axis 0
     dft_axis_kernel<true, false><<<grid, T, 0, st>>>(rho, A, c->tw[2], n2, 1u, total, 0, 1.0);
+    {   // every later launch has the same shape on the same stream: if this one was accepted the others are too,
+        // and if it was not, nothing has been enqueued
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return cuda_fail(c, e0);
+    }
     dft_axis_kernel<false, false><<<grid, T, 0, st>>>(A, B, c->tw[1], n1, n2, total, 0, 1.0);
     dft_axis_kernel<false, false><<<grid, T, 0, st>>>(B, A, c->tw[0], n0, n1 * n2, total, 0, 1.0);
     FieldArgs fa;
@@ -808,6 +847,7 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
     if (q < 1 || !(q & 1)) return BSL6D_EINVAL;
     if (partial_overlap(c, f_in, f_out)) return BSL6D_EALIAS;
     if (alpha_cells == f_out || partial_overlap(c, alpha_cells, f_out)) return BSL6D_EALIAS;
+    if (int rcd = check_device(c)) return rcd;
     const int32_t* n = c->g.n;
     size_t inner = 1, outer = 1;
     for (int d = dim + 1; d < 6; ++d) inner *= (size_t)n[d];
@@ -830,10 +870,7 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
         grid = (unsigned)((inner * outer + (size_t)pc.threads - 1) / (size_t)pc.threads);
     }
     cudaError_t e;
-    if (pc.smem > 48 * 1024) {
-        e = cudaFuncSetAttribute(pc.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pc.smem);
-        if (e != cudaSuccess) return cuda_fail(c, e);
-    }
+    if (int rcs = allow_smem(c, pc.fn, pc.smem)) return rcs;
     void* args[] = {(void*)&a};
     e = cudaLaunchKernel(pc.fn, dim3(grid), dim3(pc.threads), args, pc.smem, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
@@ -875,6 +912,14 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
     for (int i = 0; i < cnt; ++i)
         vs[nv++] = SweepDesc{sh[i].dim, c->d_nodes + c->node_off[sh[i].src_dim], 1u << sh[i].src_dim, sh[i].scale};
     for (int d = 0; d < 3; ++d) vs[nv++] = xs[d];
+    {   // plan both halves before the first launch: a failed call must not leave f half-advanced
+        if (f_tmp && (f_tmp == f || partial_overlap(c, f, f_tmp))) return BSL6D_EALIAS;
+        std::vector<Pass> dry;
+        rc = plan_passes(c, xs, 3, dry);
+        if (rc) return rc;
+        rc = plan_passes(c, vs, nv, dry);
+        if (rc) return rc;
+    }
     rc = run_sequence_pingpong(c, f, f_tmp, xs, 3, st);
     if (rc) return rc;
     rc = bsl6d_density(c, f, rho, stream);
@@ -886,6 +931,7 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
 
 int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     if (!c || !f || !rho) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
     const bsl6d_grid& g = c->g;
     const size_t seg = (size_t)g.n[3] * g.n[4] * g.n[5];
     const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
@@ -912,6 +958,7 @@ int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
 
 int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, const bsl6d_host_op* ops, int nops) {
     if (!c || !f_in_host || !f_out_host || nops < 0 || (nops > 0 && !ops)) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
     const bsl6d_grid& g = c->g;
     const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
     const size_t bytes = c->npts * sizeof(double);

@@ -46,7 +46,7 @@ struct FusedArgs {
 // One pencil: shift -> (k, theta) -> load in shifted order -> weights -> N outputs in res[].
 // GLOBAL: streaming loads from global memory; otherwise plain loads (shared memory).
 template <int N, int Q, bool PERIODIC, bool GLOBAL>
-__device__ __forceinline__ void sweep_pencil(const double* __restrict__ pin, size_t stride, double sval, double scale,
+__device__ __forceinline__ void sweep_pencil(const double* pin, size_t stride, double sval, double scale,
                                              double (&res)[N]) {
     long long k;
     double theta;

@@ -88,8 +88,8 @@ __global__ void __launch_bounds__(T, MINB) pointwise_strided_kernel(const Pointw
     const uint32_t o = p / a.inner, i = p - o * a.inner;
     const size_t stride = a.inner;
     const size_t base = (size_t)o * N * stride + i;
-    const double* __restrict__ pin = a.in + base;
-    const double* __restrict__ pal = a.alpha + base;
+    const double* pin = a.in + base;
+    const double* pal = a.alpha + base;
     double* pout = a.out + base;
     // every load of the pencil -- values and displacements -- is issued before the first store: 2N loads in flight
     // per thread, and stores to f_out can never be ordered between them (f_out may alias f_in)
@@ -117,8 +117,8 @@ __global__ void __launch_bounds__(T, MINB) pointwise_unit_kernel(const Pointwise
     const size_t p0 = (size_t)blockIdx.x * T;
     const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
     const uint32_t nelem = np * N;
-    const double* __restrict__ pin = a.in + p0 * N;
-    const double* __restrict__ pal = a.alpha + p0 * N;
+    const double* pin = a.in + p0 * N;
+    const double* pal = a.alpha + p0 * N;
     double* pout = a.out + p0 * N;
 #pragma unroll
     for (int it = 0; it < N; ++it) {

@@ -20,6 +20,8 @@
 #include <cuda_runtime.h>
 
 // Cache hints of the streaming accesses to f (every element is touched once per sweep): evict-first loads and stores.
+// f_in == f_out is legal for every sweep, so the f pointers carry no __restrict__ and BSL6D_LD must stay a coherent
+// load (never ld.global.nc / __ldg): a thread's loads of its pencil must not be moved past its stores.
 #ifndef BSL6D_LD
 #define BSL6D_LD __ldcs
 #endif
@@ -130,7 +132,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
 
     const size_t stride = a.inner;
     const size_t base = (size_t)o * N * stride + i;
-    const double* __restrict__ pin = a.in + base;
+    const double* pin = a.in + base;
     double* pout = a.out + base;
 
     constexpr int NU = PERIODIC ? N : N + Q - 1;
@@ -186,7 +188,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_unit_kernel(const SweepArgs a) 
     constexpr int NE = PB * N;                             // elements per full block
     const size_t p0 = (size_t)blockIdx.x * PB;             // first pencil of this block
     const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)PB ? ((size_t)a.outer - p0) : (size_t)PB);
-    const double* __restrict__ pin = a.in + p0 * N;
+    const double* pin = a.in + p0 * N;
     double* pout = a.out + p0 * N;
     const uint32_t nelem = np * N;
 
@@ -323,7 +325,7 @@ __global__ void __launch_bounds__(T) sweep_generic_unit_kernel(const SweepArgs a
     const size_t p0 = (size_t)blockIdx.x * T;
     const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
     const uint32_t nelem = np * (uint32_t)n;
-    const double* __restrict__ pin = a.in + p0 * n;
+    const double* pin = a.in + p0 * n;
     double* pout = a.out + p0 * n;
     for (uint32_t e = threadIdx.x; e < nelem; e += T) tin[(e / n) * LD + (e % n)] = __ldcs(pin + e);
     __syncthreads();

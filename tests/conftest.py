@@ -12,6 +12,16 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
-def pytest_collection_modifyitems(config, items):
-    """GPU tests fail loudly (not skip) when selected on a box without a device or without the library."""
-    return
+def need_gpu(free_gib: float = 0.0):
+    """GPU tests fail loudly (never skip) when selected on a box without a device or with too little free device
+    memory: a full-size parity check that silently vanishes would leave the GPU suite green for the wrong reason."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("this test is marked gpu and needs a CUDA device (run with -m 'not gpu' on a CPU box)",
+                    pytrace=False)
+    if free_gib > 0.0:
+        torch.cuda.empty_cache()
+        free, _ = torch.cuda.mem_get_info()
+        if free < free_gib * 2 ** 30:
+            pytest.fail(f"needs {free_gib} GiB of free device memory, only {free / 2 ** 30:.1f} GiB are free",
+                        pytrace=False)

@@ -25,11 +25,8 @@ TOL = 1e-12
 
 
 def _need(gb: float):
-    if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
-    free, _ = torch.cuda.mem_get_info()
-    if free < gb * 2 ** 30:
-        pytest.skip(f"needs {gb} GiB of free device memory")
+    from conftest import need_gpu
+    need_gpu(gb)
 
 
 def _split(w, dim):

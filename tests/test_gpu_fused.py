@@ -18,8 +18,8 @@ TOL = 1e-12
 
 
 def _need_gpu():
-    if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
+    from conftest import need_gpu
+    need_gpu()
 
 
 def ogrid(w):

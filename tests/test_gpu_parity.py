@@ -242,6 +242,58 @@ def test_rotation_each_axis(axis):
         assert torch.equal(z, g)
 
 
+@pytest.mark.parametrize("axis", (0, 1, 2))
+@pytest.mark.parametrize("theta", (3.0, -2.0, 6.2))
+def test_rotation_large_angle_each_axis(axis, theta):
+    """Reading R2: an axis rotation above pi/2 runs in equal pieces (the library and the oracle plan it alike);
+    more than a full turn is BSL6D_EUNSUPPORTED."""
+    _need_gpu()
+    w = wl.C4.reduced((2, 3, 2, 32, 32, 32))
+    f = w.make_f("cpu").numpy()
+    B = [0.0, 0.0, 0.0]
+    B[axis] = theta / 0.5
+    with ctx_for(w) as ctx:
+        out = torch.empty_like(dev(f))
+        ctx.rotate(dev(f), out, B, 0.5)
+        assert_close(out, oracle.rotate(ogrid(w), w.degree, f, B, 0.5), f"rotate axis {axis} by {theta}")
+        assert float(out.abs().max()) > 0.05                  # not shorn off the grid
+        ctx.set_fusion(0)
+        out2 = torch.empty_like(out)
+        ctx.rotate(dev(f), out2, B, 0.5)
+        assert torch.equal(out, out2)
+        B[axis] = 13.0
+        with pytest.raises(bsl.Bsl6dError) as ei:
+            ctx.rotate(dev(f), out, B, 0.5)
+        assert ei.value.code == bsl.EUNSUPPORTED
+
+
+def test_binding_checks_counts_and_device():
+    """api.py validates what the C ABI cannot see: element counts of every tensor argument."""
+    _need_gpu()
+    w = wl.C1
+    f = dev(w.make_f("cpu").numpy())
+    out = torch.empty_like(f)
+    nx = w.n[0] * w.n[1] * w.n[2]
+    good_E = [torch.zeros(nx, dtype=torch.float64, device="cuda") for _ in range(3)]
+    bad = torch.zeros(nx - 1, dtype=torch.float64, device="cuda")
+    with ctx_for(w) as ctx:
+        with pytest.raises(ValueError):
+            ctx.advect(f, out, 0, bad, 0.1)                  # x sweep wants n[3] values
+        with pytest.raises(ValueError):
+            ctx.advect(f, out, 3, bad, 0.1)                  # v sweep wants nx values
+        with pytest.raises(ValueError):
+            ctx.strang_step(f, out[..., :-1].contiguous(), good_E, None, 0.1)
+        with pytest.raises(ValueError):
+            ctx.strang_step(f, None, [good_E[0], bad, good_E[2]], None, 0.1)
+        with pytest.raises(ValueError):
+            ctx.advect_seq(f, out, [(3, bad, 0x7, 1.0)])
+        with pytest.raises(ValueError):
+            ctx.density(f, bad)
+        with pytest.raises(ValueError):
+            ctx.field_poisson(bad, 1.0, 1.0, good_E)
+        ctx.advect(f, out, 3, good_E[0], 0.1)                # and the well-formed call still goes through
+
+
 def test_C4_reduced_rotation_return_63_steps():
     """configs[3] at reduced x extent, full depth: 63 steps of theta = 2*pi/63 (reading S7), GPU == oracle
     after all 189 sweeps, and both return to the start within interpolation error."""

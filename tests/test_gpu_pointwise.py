@@ -14,10 +14,8 @@ TOL = 1e-12
 
 
 def _need(gb=0.0):
-    if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
-    if gb and torch.cuda.mem_get_info()[0] < gb * 2 ** 30:
-        pytest.skip(f"needs {gb} GiB of free device memory")
+    from conftest import need_gpu
+    need_gpu(gb)
 
 
 def _ctx(n):

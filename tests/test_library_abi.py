@@ -42,11 +42,29 @@ def test_no_compute_symbols_needed_on_cpu(lib):
 
 
 def test_sass_is_sm100a_fp64_fma():
-    """The shipped cubin targets sm_100a and the sweep kernels are plain fp64 FMA code (no tensor-core path)."""
-    r = subprocess.run(["cuobjdump", "-lelf", bsl.LIB_PATH], capture_output=True, text=True)
-    if r.returncode != 0:
-        pytest.skip("cuobjdump not available")
-    assert "sm_100a" in r.stdout
+    """The shipped cubins target sm_100a, the sweep kernels are fp64 FMA code (DFMA) with no tensor-core path
+    (no UTC*MMA / HMMA: the op is a bandwidth-bound stencil, north_star), and nothing spills to local memory in
+    the kernels the benchmark times."""
+    exe = "/usr/local/cuda/bin/cuobjdump"
+    r = subprocess.run([exe, "-lelf", bsl.LIB_PATH], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    elfs = [ln for ln in r.stdout.splitlines() if ".cubin" in ln]
+    assert elfs and all("sm_100a" in ln for ln in elfs), r.stdout
+    r = subprocess.run([exe, "-sass", bsl.LIB_PATH], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    sass = r.stdout
+    assert sass.count("DFMA") > 1000                          # the q-term dot products
+    for bad in ("HMMA", "UTCHMMA", "UTCQMMA", "HGMMA", "IMMA", "DMMA"):
+        assert bad not in sass, bad
+    # per-function check: the specialised sweep kernels keep their pencil in registers (no local-memory traffic)
+    fn, bad_fns = None, set()
+    for ln in sass.splitlines():
+        s = ln.strip()
+        if s.startswith("Function :"):
+            fn = s.split(":", 1)[1].strip()
+        elif fn and ("sweep_strided_kernel" in fn or "sweep_unit_kernel" in fn) and (" LDL" in s or " STL" in s):
+            bad_fns.add(fn)
+    assert not bad_fns, sorted(bad_fns)[:3]
 
 
 def test_product_path_does_not_import_oracle():

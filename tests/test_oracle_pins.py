@@ -339,6 +339,46 @@ def test_rotation_closed_form(axis, theta):
     assert wrong > 0.05                                 # the other rotation sense is far away
 
 
+@pytest.mark.parametrize("axis", (0, 1, 2))
+@pytest.mark.parametrize("theta", (3.0, -2.0, 6.0))
+def test_rotation_large_angle_closed_form(axis, theta):
+    """Reading R2: an axis rotation above pi/2 runs in equal pieces of three shears (tan(theta/2) diverges at pi).
+    Pinned by the closed-form image of an off-centre blob; one unsplit three-shear rotation at theta = 3 would
+    push the blob off the grid (tan 1.5 = 14 cells of shear per cell)."""
+    a, b = (axis + 1) % 3, (axis + 2) % 3
+    B = [0.0, 0.0, 0.0]; B[axis] = theta / 0.5
+    c, s = math.cos(theta), math.sin(theta)
+    blob = lambda x, y: _blob(x, y, c=(0.8, 0.3), sig=0.6)   # stays inside [-6,6]^2 under shears of tan(pi/4) = 1
+    errs = {}
+    for nv in (64, 128):
+        n = [1, 1, 1, 1, 1, 1]
+        n[3 + a] = n[3 + b] = nv
+        g = small_grid(n, vmax=6.0)
+        va, vb = g.nodes(3 + a), g.nodes(3 + b)
+        sa, sb = [1] * 6, [1] * 6
+        sa[3 + a] = nv; sb[3 + b] = nv
+        VA, VB = va.reshape(sa), vb.reshape(sb)
+        f0 = np.ascontiguousarray(np.broadcast_to(blob(VA, VB), n))
+        out = oracle.rotate(g, 7, f0, B, 0.5)
+        errs[nv] = np.max(np.abs(out - blob(c * VA - s * VB, s * VA + c * VB)))
+        wrong = np.max(np.abs(out - blob(c * VA + s * VB, -s * VA + c * VB)))
+        assert wrong > 0.05                             # the other rotation sense is far away
+    assert errs[64] < 1e-4 and errs[128] < 1e-6 and errs[64] / errs[128] > 50, errs   # order ~ q = 8
+    # the pieces compose: the same turn as explicit equal pieces, bit for bit
+    pieces = int(math.ceil(abs(theta) / (math.pi / 2)))
+    f = f0
+    for _ in range(pieces):
+        f = oracle.rotate(g, 7, f, [x / pieces for x in B], 0.5)
+    assert np.array_equal(f, out)
+
+
+def test_rotation_about_an_axis_rejects_more_than_a_full_turn():
+    g = small_grid([1, 1, 1, 8, 8, 8])
+    f = np.random.default_rng(0).random(g.n)
+    with pytest.raises(ValueError):
+        oracle.rotate(g, 7, f, [0.0, 0.0, 13.0], 0.5)
+
+
 def _rotation_return_error(nv, q, nsteps=63):
     g = small_grid([1, 1, 1, nv, nv, 1], vmax=6.0)
     v1, v2 = g.nodes(3)[:, None], g.nodes(4)[None, :]
