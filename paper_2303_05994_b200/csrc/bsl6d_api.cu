@@ -15,6 +15,7 @@
 #include "fused_kernels.cuh"
 #include "pointwise_kernels.cuh"
 #include "sweep_kernels.cuh"
+#include "vblock_kernels.cuh"
 
 using bsl6d::SweepArgs;
 
@@ -35,6 +36,8 @@ struct bsl6d_ctx {
     int field_ready;          // field step: every table and work array is allocated
     int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
+    int vblock_min;           // fewest sweeps a whole-v-block pass is used for
+    int use_vblock;           // 1: runs of velocity-space sweeps run as one whole-v-block pass where a kernel exists
     const void* smem_ok[64];  // kernels whose dynamic shared-memory limit has been raised (and to how much)
     size_t smem_ok_bytes[64];
     int n_smem_ok;
@@ -338,9 +341,11 @@ struct SweepDesc { int dim; const double* src; unsigned mask; double scale; };
 
 struct Pass {
     int first, count;         // sweeps [first, first+count)
-    bool fused;
+    bool fused;               // two-dim tile pass (fused_kernels.cuh)
     bsl6d::FusedChoice fc;
     int pattern;
+    bool vblock;              // whole-v-block pass (vblock_kernels.cuh)
+    bsl6d::VBlockChoice vc;
 };
 
 bool fused_lookup(int q, int na, int nb, bool pa, bool pb, int pattern, bsl6d::FusedChoice& fc) {
@@ -384,7 +389,21 @@ bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) 
     }
     const size_t blocks = outer * mid * (inner_b / (size_t)fc.C);
     if (blocks > 0x7FFFFFFFull) return false;
-    p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern;
+    p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern; p.vblock = false;
+    return true;
+}
+
+// Can sweeps [i, i+cnt) -- all of them along velocity dims -- run as one whole-v-block pass?
+bool try_vblock(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) {
+    if (cnt < 2 || cnt > bsl6d::kMaxVSweeps) return false;
+    for (int k = 0; k < cnt; ++k)
+        if (sw[i + k].dim < 3) return false;
+    const int32_t* n = c->g.n;
+    bsl6d::VBlockChoice vc;
+    if (!bsl6d::vblock_lookup(n[3], n[4], n[5], c->q, vc)) return false;
+    const size_t nx = (size_t)n[0] * n[1] * n[2];
+    if (c->npts > 0xFFFFFFFFull || nx * (size_t)vc.cl > 0x7FFFFFFFull) return false;
+    p.first = i; p.count = cnt; p.fused = false; p.pattern = 0; p.vblock = true; p.vc = vc;
     return true;
 }
 
@@ -398,25 +417,34 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
         if (rc) return rc;
     }
     // Fewest passes over the chain (dynamic programme from the back): a group of 3 (a,b,a), 2 (a,b) or 1 sweeps.
+    // pick[i] > 0: a two-dim tile pass over that many sweeps (or a single sweep); pick[i] < 0: a whole-v-block pass
+    // over -pick[i] sweeps.  Ties go to the later candidate: v-block pass > triple > pair > single.
     std::vector<int> best(ns + 1, 0), pick(ns + 1, 1);
-    std::vector<Pass> cand2(ns), cand3(ns);
-    std::vector<char> ok2(ns, 0), ok3(ns, 0);
+    std::vector<Pass> cand2(ns), cand3(ns), candv(ns);
     for (int i = ns - 1; i >= 0; --i) {
         best[i] = 1 + best[i + 1];
         pick[i] = 1;
         if (c->fusion && i + 1 < ns && try_fuse(c, sw, i, 2, cand2[i])) {
-            ok2[i] = 1;
             if (1 + best[i + 2] < best[i]) { best[i] = 1 + best[i + 2]; pick[i] = 2; }
         }
         if (c->fusion && i + 2 < ns && try_fuse(c, sw, i, 3, cand3[i])) {
-            ok3[i] = 1;
             if (1 + best[i + 3] < best[i]) { best[i] = 1 + best[i + 3]; pick[i] = 3; }
         }
+        if (c->fusion && c->use_vblock) {
+            int run = 0;
+            while (i + run < ns && sw[i + run].dim >= 3 && run < bsl6d::kMaxVSweeps) ++run;
+            for (int len = c->vblock_min; len <= run; ++len) {
+                Pass p;
+                if (!try_vblock(c, sw, i, len, p)) break;
+                if (1 + best[i + len] <= best[i]) { best[i] = 1 + best[i + len]; pick[i] = -len; candv[i] = p; }
+            }
+        }
     }
-    for (int i = 0; i < ns; i += pick[i]) {
-        if (pick[i] == 3) passes.push_back(cand3[i]);
+    for (int i = 0; i < ns; i += (pick[i] < 0 ? -pick[i] : pick[i])) {
+        if (pick[i] < 0) passes.push_back(candv[i]);
+        else if (pick[i] == 3) passes.push_back(cand3[i]);
         else if (pick[i] == 2) passes.push_back(cand2[i]);
-        else passes.push_back(Pass{i, 1, false, {}, 0});
+        else passes.push_back(Pass{i, 1, false, {}, 0, false, {}});
     }
     return BSL6D_OK;
 }
@@ -455,7 +483,32 @@ int launch_fused(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDes
     return BSL6D_OK;
 }
 
+int launch_vblock(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDesc* sw, const Pass& p,
+                  cudaStream_t stream) {
+    const int32_t* n = c->g.n;
+    bsl6d::VBlockArgs va;
+    std::memset(&va, 0, sizeof(va));
+    va.nsweeps = (uint32_t)p.count;
+    va.nx = (uint32_t)((size_t)n[0] * n[1] * n[2]);
+    for (int k = 0; k < p.count; ++k) {
+        const SweepDesc& s = sw[p.first + k];
+        va.sw[k].src = s.src;
+        va.sw[k].scale = s.scale;
+        va.sw[k].dim = s.dim;
+        int rc = build_src_terms(n, s.dim, s.mask, va.sw[k].terms);
+        if (rc) return rc;
+    }
+    if (int rcs = allow_smem(c, p.vc.fn, p.vc.smem)) return rcs;
+    cudaError_t e = bsl6d::vblock_launch(p.vc, f_in, f_out, va.nx, n[3], va, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
+}
+
 int launch_pass(bsl6d_ctx* c, const double* src, double* dst, const SweepDesc* sw, const Pass& p, cudaStream_t st) {
+    if (p.vblock) return launch_vblock(c, src, dst, sw, p, st);
     if (p.fused) return launch_fused(c, src, dst, sw, p, st);
     const SweepDesc& s = sw[p.first];
     return launch_sweep(c, src, dst, s.dim, s.src, s.mask, s.scale, st);
@@ -686,6 +739,8 @@ int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
     c->npts = npts;
     c->fusion = 1;
     c->fuse_all = 0;
+    c->use_vblock = 1;
+    c->vblock_min = 2;
 
     std::vector<double> nodes(nn);
     size_t off = 0;
@@ -835,9 +890,11 @@ int bsl6d_seq_passes(bsl6d_ctx* c, const bsl6d_sweep* sweeps, int nsweeps) {
 
 int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     if (!c) return BSL6D_EINVAL;
-    const int old = c->fusion ? (c->fuse_all ? 2 : 1) : 0;
+    if (enable < 0 || enable > 3) return BSL6D_EINVAL;
+    const int old = !c->fusion ? 0 : (c->fuse_all ? 2 : (c->use_vblock ? 1 : 3));
     c->fusion = enable ? 1 : 0;
     c->fuse_all = enable == 2 ? 1 : 0;
+    c->use_vblock = enable == 3 ? 0 : 1;
     return old;
 }
 

@@ -20,6 +20,25 @@ bool fused_lookup_q10(int na, int nb, bool pa, bool pb, int pattern, FusedChoice
 
 }  // namespace bsl6d
 
+// ---- whole-v-block passes (vblock_kernels.cuh, bsl6d_vblock.cu) ----------------------------------------------------
+#include <cstdint>
+#include <cuda_runtime.h>
+namespace bsl6d {
+struct VBlockArgs;
+struct VBlockChoice {
+    const void* fn;        // __global__ void (*)(CUtensorMap, CUtensorMap, VBlockArgs)
+    int threads;
+    size_t smem;
+    int cl;                // CTAs per cluster = CTAs per v-block
+    int cw;                // v3 columns per CTA
+};
+// Is there a whole-v-block kernel for a cubic velocity grid nv^3 and stencil width q (and a TMA-capable driver)?
+bool vblock_lookup(int nv1, int nv2, int nv3, int q, VBlockChoice& out);
+// Encode the tensor maps of f_in / f_out ([nx][nv][nv][nv] doubles) and enqueue one pass.
+cudaError_t vblock_launch(const VBlockChoice& vc, const double* f_in, double* f_out, uint32_t nx, int nv,
+                          const VBlockArgs& args, cudaStream_t stream);
+}  // namespace bsl6d
+
 // ---- pointwise (odd q, per-point displacement) kernels, bsl6d_pointwise.cu -------------------------------------
 namespace bsl6d {
 struct PointwiseChoice {

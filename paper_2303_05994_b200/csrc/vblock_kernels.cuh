@@ -1,0 +1,245 @@
+// vblock_kernels.cuh -- SURVEY.md 8(f) N1: EVERY velocity-space sweep of a step in ONE pass over f (sm_100a).
+//
+// In C order each x-point owns one contiguous block of nv1*nv2*nv3 doubles (256 KB at 32^3), and the whole v-part of
+// the Lie chain -- the three E-sweeps v1,v2,v3 and the shears of the rotation -- acts inside it.
+// A thread-block CLUSTER of CL CTAs stages one x-point's v-block on chip, cut along v3: CTA r holds
+//     tile[j1][j2][c],  c = 0..CW-1  <->  j3 = r*CW + c,   CW = NV/CL      (64 KB per CTA at 32^3 with CL = 4)
+// fetched by ONE TMA bulk-tensor copy (cp.async.bulk.tensor.4d + mbarrier; no register staging), and written back
+// by one TMA store.  All sweeps run in place in shared memory: HBM traffic is 16 B/point for the whole group.
+//
+//   v1 / v2 sweeps  thread owns the pencil (j2,c) / (j1,c): whole pencil -> registers in shifted order ->
+//                   Q-term FMA chains -> back into the tile.  Entirely CTA-local.
+//   v3 sweeps       the pencil crosses the cluster.  Thread owns row pieces (j1,j2, this CTA's CW outputs); the
+//                   CW+Q-1 inputs are read through distributed shared memory (mapa + ld.shared::cluster) from
+//                   whichever CTA owns the column; cluster barriers separate "everyone has read" from "write".
+//
+// The tile rows are CW*8 = 64 or 128 bytes, written by the TMA with the matching 64B / 128B swizzle (16-byte chunk
+// index XOR row bits), which is what makes the v3 sweeps (lanes along rows) and the v1/v2 sweeps (lanes along c)
+// both bank-conflict-light without padding -- TMA boxes cannot be padded.
+// Per sweep the arithmetic (split_shift, lagrange_weights, the fma chain) is that of sweep_kernels.cuh, so a pass is
+// bit-identical to the same sweeps launched one by one.
+#pragma once
+#include <cuda.h>
+#include <cooperative_groups.h>
+
+#include "sweep_kernels.cuh"
+
+namespace bsl6d {
+
+constexpr int kMaxVSweeps = 12;
+
+struct VSweep {
+    const double* src;
+    double scale;
+    int32_t dim;           // 3, 4 or 5
+    SrcTerms terms;        // in terms of the (outer, inner) index of that sweep's own [outer][N][inner] view
+};
+
+struct VBlockArgs {
+    uint32_t nsweeps;
+    uint32_t nx;           // number of x-points = number of v-blocks
+    VSweep sw[kMaxVSweeps];
+};
+
+namespace vb {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "DONE:\n\t"
+        "}" ::"r"(bar), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* map, uint32_t src, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(map),
+                 "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts_f64(uint32_t addr, double v) {
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+// read a double of CTA `rank`'s shared memory at this CTA's address `addr` (distributed shared memory)
+__device__ __forceinline__ double ld_cluster_f64(uint32_t addr, uint32_t rank) {
+    uint32_t ra;
+    double v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(addr), "r"(rank));
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(ra));
+    return v;
+}
+
+// Outputs j0 .. j0+NOUT-1 of a zero-extended pencil of N points: load the NOUT+Q-1 inputs in shifted order through
+// `ld(row)` (row in [0,N) guaranteed), weights, FMA chains -- the arithmetic of sweep_pencil<N,Q,false,...>.
+template <int N, int NOUT, int Q, class Load>
+__device__ __forceinline__ void window_sweep(double sval, double scale, int j0, Load&& ld, double (&res)[NOUT]) {
+    long long k;
+    double theta;
+    split_shift(sval, scale, k, theta);
+    long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
+    kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
+    const int r0 = (int)kc + (1 - Q / 2) + j0;
+    constexpr int NU = NOUT + Q - 1;
+    double u[NU];
+#pragma unroll
+    for (int t = 0; t < NU; ++t) {
+        const int row = r0 + t;
+        double v = 0.0;
+        if (row >= 0 && row < N) v = ld(row);
+        u[t] = v;
+    }
+    double w[Q];
+    lagrange_weights<Q>(theta, w);
+#pragma unroll
+    for (int j = 0; j < NOUT; ++j) {
+        double acc = w[0] * u[j];
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[j + m], acc);
+        res[j] = acc;
+    }
+}
+
+}  // namespace vb
+
+template <int NV, int CL>
+struct VBlockGeom {
+    static constexpr int CW = NV / CL;                     // columns (v3 values) per CTA
+    static constexpr int RB = CW * 8;                      // tile row bytes: 64 or 128 (= the TMA swizzle span)
+    static constexpr uint32_t SWZ = RB == 128 ? 7u : 3u;   // 16-byte chunk index ^= row bits & SWZ
+    static constexpr int PLANE = NV * RB;                  // bytes per j1 plane
+    static constexpr int TILE = NV * PLANE;                // bytes per CTA tile
+    static constexpr int T = NV * CW < 256 ? (NV * CW < 32 ? 32 : NV * CW) : 256;   // threads per CTA
+    static constexpr size_t kSmemBytes = (size_t)TILE + 1024;   // + alignment slack (swizzle pattern repeats at 1 KB)
+    static_assert(NV % CL == 0 && (RB == 64 || RB == 128), "tile rows must be 64 or 128 bytes");
+    static_assert(PLANE % 1024 == 0 || (RB == 64 && PLANE % 512 == 0), "j1 planes must not disturb the swizzle bits");
+};
+
+template <int NV, int Q, int CL, int MINB>
+__global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__((VBlockGeom<NV, CL>::T), MINB)
+    vblock_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out,
+                  const __grid_constant__ VBlockArgs a) {
+    using G = VBlockGeom<NV, CL>;
+    constexpr int CW = G::CW, RB = G::RB, PLANE = G::PLANE, T = G::T;
+    constexpr uint32_t SWZ = G::SWZ;
+    extern __shared__ unsigned char vb_smem_raw[];
+    __shared__ __align__(8) unsigned long long vb_mbar;
+    const uint32_t tile = (vb::smem_u32(vb_smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar = vb::smem_u32(&vb_mbar);
+    const uint32_t rank = CL > 1 ? (blockIdx.x % CL) : 0u;
+    const uint32_t x = blockIdx.x / CL;
+    const int c_lo = (int)rank * CW;                       // first v3 index of this CTA
+
+    if (threadIdx.x == 0) {
+        vb::mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        vb::mbar_expect_tx(bar, (uint32_t)G::TILE);
+        vb::tma_load_4d(tile, &tm_in, bar, c_lo, 0, 0, (int)x);
+    }
+    vb::mbar_wait(bar, 0);
+
+    for (uint32_t s = 0; s < a.nsweeps; ++s) {
+        const VSweep& sw = a.sw[s];
+        if (sw.dim == 3) {
+            // ---- along v1: pencil (j2, c), element j1 at  p_off + j1*PLANE  (swizzle term does not depend on j1)
+            for (int p = threadIdx.x; p < NV * CW; p += T) {
+                const uint32_t j2 = p / CW, c = p % CW;
+                const uint32_t off = j2 * RB + c * 8;
+                const uint32_t base = tile + (off ^ (((off >> 7) & SWZ) << 4));
+                const double sval = __ldg(sw.src + src_offset(sw.terms, x, j2 * NV + (uint32_t)c_lo + c));
+                double res[NV];
+                vb::window_sweep<NV, NV, Q>(sval, sw.scale, 0,
+                                            [&](int row) { return vb::lds_f64(base + (uint32_t)row * PLANE); }, res);
+#pragma unroll
+                for (int j = 0; j < NV; ++j) vb::sts_f64(base + (uint32_t)j * PLANE, res[j]);
+            }
+        } else if (sw.dim == 4) {
+            // ---- along v2: pencil (j1, c), element j2 at  j1*PLANE + swz(j2*RB + c*8)
+            for (int p = threadIdx.x; p < NV * CW; p += T) {
+                const uint32_t j1 = p / CW, c = p % CW;
+                const uint32_t base = tile + j1 * PLANE;
+                const uint32_t c8 = c * 8;
+                const double sval = __ldg(sw.src + src_offset(sw.terms, x * NV + j1, (uint32_t)c_lo + c));
+                double res[NV];
+                vb::window_sweep<NV, NV, Q>(sval, sw.scale, 0,
+                                            [&](int row) {
+                                                const uint32_t o = (uint32_t)row * RB;
+                                                return vb::lds_f64(base + o + (c8 ^ (((o >> 7) & SWZ) << 4)));
+                                            },
+                                            res);
+#pragma unroll
+                for (int j = 0; j < NV; ++j) {
+                    const uint32_t o = (uint32_t)j * RB;   // compile-time
+                    vb::sts_f64(base + o + (c8 ^ (((o >> 7) & SWZ) << 4)), res[j]);
+                }
+            }
+        } else {
+            // ---- along v3: row piece (j1, j2) x this CTA's CW outputs; inputs from any CTA of the cluster
+            constexpr int RP = (NV * NV + T - 1) / T;      // row pieces per thread
+            double res[RP][CW];
+            if (CL > 1) cooperative_groups::this_cluster().sync();     // the previous sweep's writes, cluster-wide
+#pragma unroll
+            for (int r = 0; r < RP; ++r) {
+                const uint32_t p = r * T + threadIdx.x;    // row = j1*NV + j2
+                if (p < NV * NV) {
+                    const uint32_t roff = p * RB;
+                    const uint32_t rbase = tile + roff;
+                    const uint32_t sx = ((roff >> 7) & SWZ) << 4;
+                    const double sval = __ldg(sw.src + src_offset(sw.terms, x * (NV * NV) + p, 0u));
+                    vb::window_sweep<NV, CW, Q>(sval, sw.scale, c_lo,
+                                                [&](int col) {
+                                                    const uint32_t owner = (uint32_t)col / CW, cl = (uint32_t)col % CW;
+                                                    const uint32_t ad = rbase + ((cl * 8) ^ sx);
+                                                    return CL > 1 ? vb::ld_cluster_f64(ad, owner) : vb::lds_f64(ad);
+                                                },
+                                                res[r]);
+                }
+            }
+            if (CL > 1) cooperative_groups::this_cluster().sync();     // every CTA has read what it needs
+#pragma unroll
+            for (int r = 0; r < RP; ++r) {
+                const uint32_t p = r * T + threadIdx.x;
+                if (p < NV * NV) {
+                    const uint32_t roff = p * RB;
+                    const uint32_t sx = ((roff >> 7) & SWZ) << 4;
+#pragma unroll
+                    for (int j = 0; j < CW; ++j) vb::sts_f64(tile + roff + (((uint32_t)j * 8) ^ sx), res[r][j]);
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // generic-proxy writes -> visible to the async proxy, then one bulk store of the tile
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        vb::tma_store_4d(&tm_out, tile, c_lo, 0, 0, (int)x);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    }
+}
+
+}  // namespace bsl6d

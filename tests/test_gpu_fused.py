@@ -165,7 +165,7 @@ def test_sequence_error_paths_enqueue_nothing():
     _need_gpu()
     w = wl.C1
     fd = w.make_f("cuda")
-    one = torch.ones(1, dtype=torch.float64, device="cuda")
+    one = torch.ones(w.n[1], dtype=torch.float64, device="cuda")   # sized for the mask, so the C check is what fires
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
         with pytest.raises(bsl.Bsl6dError) as e:
             ctx.advect_seq(fd, fd, [(0, None, 0, 0.1), (3, None, 0x7, 0.1)])   # v sweep without a source
