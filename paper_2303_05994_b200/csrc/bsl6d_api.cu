@@ -57,7 +57,7 @@ struct KernelChoice {
     int threads;
     size_t smem;
     int kind;                 // 0 strided, 1 unit, 2 generic
-    int gen_T;                // generic: threads; unit: segments per pencil S
+    int gen_T;                // generic: threads; unit and strided: segments per pencil S
 };
 
 // Launch shape of the strided sweep: T threads per block, at least MINB resident blocks per SM (caps the
@@ -75,11 +75,23 @@ constexpr int strided_minblocks() {
 }
 #endif
 
+// Segments per pencil: 1 (a thread owns its whole pencil) unless the pencil is too long for 4 blocks per SM.
+#ifdef BSL6D_TUNE_SS
+template <int N, int Q, bool P> constexpr int strided_segments() { return (N >= 48 && N % BSL6D_TUNE_SS == 0 && N / BSL6D_TUNE_SS >= Q) ? BSL6D_TUNE_SS : 1; }
+#else
+template <int N, int Q, bool P> constexpr int strided_segments() { return 1; }
+#endif
+
 template <int N, int Q, bool P>
 KernelChoice strided_choice() {
+    constexpr int S = strided_segments<N, Q, P>();
     constexpr int T = strided_threads<N, Q, P>();
-    constexpr int MINB = strided_minblocks<N, Q, P>();
-    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB>, T, 0, 0, 0};
+#ifdef BSL6D_TUNE_SMINB
+    constexpr int MINB = S == 1 ? strided_minblocks<N, Q, P>() : BSL6D_TUNE_SMINB;
+#else
+    constexpr int MINB = S == 1 ? strided_minblocks<N, Q, P>() : 4;
+#endif
+    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S};
 }
 
 // Launch shape of the unit-stride sweep: S segments per pencil, T threads (a multiple of 32*S), MINB blocks/SM.
@@ -303,9 +315,11 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
         const size_t pb = (size_t)kc.threads / (size_t)kc.gen_T;      // pencils per block = T / S
         grid = (unsigned)((outer + pb - 1) / pb);
     } else {
-        const uint64_t lim = inner < (uint64_t)kc.threads ? inner : (uint64_t)kc.threads;
+        // strided: kc.gen_T = segments per pencil (threads / segments pencils per block); generic: gen_T = threads
+        const uint64_t pencils = kc.kind == 0 ? (uint64_t)kc.threads / (uint64_t)kc.gen_T : (uint64_t)kc.threads;
+        const uint64_t lim = inner < pencils ? inner : pencils;
         a.ti_log2 = ceil_pow2_log2(lim);
-        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)kc.threads / TI;
+        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)pencils / TI;
         a.nib = (uint32_t)((inner + TI - 1) / TI);
         const uint64_t nbo = (outer + TO - 1) / TO;
         if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
@@ -396,8 +410,13 @@ bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) 
 // Can sweeps [i, i+cnt) -- all of them along velocity dims -- run as one whole-v-block pass?
 bool try_vblock(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) {
     if (cnt < 2 || cnt > bsl6d::kMaxVSweeps) return false;
-    for (int k = 0; k < cnt; ++k)
+    for (int k = 0; k < cnt; ++k) {
         if (sw[i + k].dim < 3) return false;
+        // Policy from measurement: a v3 sweep inside the pass crosses the cluster through
+        // distributed shared memory (~16 B/clk per SM at best, ~3 clk per scattered 8-byte request) and costs more
+        // than the v3 sweep as a pass of its own; only fusion mode 2 takes it.
+        if (sw[i + k].dim == 5 && !c->fuse_all) return false;
+    }
     const int32_t* n = c->g.n;
     bsl6d::VBlockChoice vc;
     if (!bsl6d::vblock_lookup(n[3], n[4], n[5], c->q, vc)) return false;
@@ -432,7 +451,9 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
         }
         if (c->fusion && c->use_vblock) {
             int run = 0;
-            while (i + run < ns && sw[i + run].dim >= 3 && run < bsl6d::kMaxVSweeps) ++run;
+            while (i + run < ns && sw[i + run].dim >= 3 && (c->fuse_all || sw[i + run].dim != 5) &&
+                   run < bsl6d::kMaxVSweeps)
+                ++run;
             for (int len = c->vblock_min; len <= run; ++len) {
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
@@ -799,6 +820,9 @@ int bsl6d_kernel_name(const bsl6d_ctx* c, int dim, char* buf, int buflen) {
     const char* kind = k.kind == 0 ? "strided" : (k.kind == 1 ? "unit" : "generic");
     if (k.kind == 1)
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q, k.gen_T, k.threads);
+    else if (k.kind == 0 && k.gen_T > 1)
+        std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q,
+                      dim < 3 ? "periodic" : "zero", k.gen_T, k.threads);
     else
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
                       dim < 3 ? "periodic" : "zero", k.threads);

@@ -117,56 +117,72 @@ __device__ __forceinline__ uint32_t src_offset(const SrcTerms& a, uint32_t o, ui
 }
 
 // ---- a4: strided sweep, one column per thread, no shared memory --------------------------------------------
-template <int N, int Q, bool PERIODIC, int T, int MINB>
+// S > 1 cuts a pencil into S segments of R = N/S outputs, one thread each (the threads of a pencil sit in different
+// warps of the same block): a thread then holds R+Q-1 instead of N values, which keeps long pencils with wide
+// stencils (N = 48, Q = 10) under the register budget of 4 resident blocks per SM.  The Q-1 rows two neighbouring
+// segments share are loaded by both threads (L1/L2 hits, never HBM); a block barrier between the load and the store
+// phase keeps f_in == f_out legal.
+template <int N, int Q, bool PERIODIC, int T, int MINB, int S = 1>
 __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs a) {
+    static_assert(N % S == 0 && T % S == 0, "segments must tile the pencil and the block");
+    constexpr int TP = T / S;                              // pencils per block
+    constexpr int R = N / S;                               // outputs per thread
+    const uint32_t tp = S == 1 ? threadIdx.x : threadIdx.x % TP;
+    const int seg = S == 1 ? 0 : (int)(threadIdx.x / TP);
     const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
     const uint32_t bo = blockIdx.x / a.nib;
     const uint32_t bi = blockIdx.x - bo * a.nib;
-    const uint32_t i = (bi << a.ti_log2) + (threadIdx.x & ti_mask);
-    const uint32_t o = bo * (T >> a.ti_log2) + (threadIdx.x >> a.ti_log2);
-    if (i >= a.inner || o >= a.outer) return;
+    const uint32_t i = (bi << a.ti_log2) + (tp & ti_mask);
+    const uint32_t o = bo * (TP >> a.ti_log2) + (tp >> a.ti_log2);
+    const bool live = i < a.inner && o < a.outer;
+    if (S == 1 && !live) return;
 
-    long long k;
-    double theta;
-    split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
+    long long k = 0;
+    double theta = 0.0;
+    if (live) split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
 
     const size_t stride = a.inner;
     const size_t base = (size_t)o * N * stride + i;
     const double* pin = a.in + base;
     double* pout = a.out + base;
 
-    constexpr int NU = PERIODIC ? N : N + Q - 1;
+    constexpr int NU = (PERIODIC && S == 1) ? N : R + Q - 1;
+    static_assert(NU <= N || !PERIODIC, "a segment's window must not wrap onto itself");
     double u[NU];
-    if (PERIODIC) {
-        int r0 = (int)((k + (long long)(1 - Q / 2)) % (long long)N);
-        if (r0 < 0) r0 += N;
+    if (live) {
+        if (PERIODIC) {
+            int r0 = (int)((k + (long long)(1 - Q / 2 + seg * R)) % (long long)N);
+            if (r0 < 0) r0 += N;
 #pragma unroll
-        for (int t = 0; t < N; ++t) {
-            int row = r0 + t;
-            if (row >= N) row -= N;
-            u[t] = BSL6D_LD(pin + (size_t)row * stride);
-        }
-    } else {
-        // rows r0 .. r0+N+Q-2; anything outside [0,N) is the zero extension
-        long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
-        kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
-        const int r0 = (int)kc + (1 - Q / 2);
+            for (int t = 0; t < NU; ++t) {
+                int row = r0 + t;
+                if (row >= N) row -= N;
+                u[t] = BSL6D_LD(pin + (size_t)row * stride);
+            }
+        } else {
+            // rows r0 .. r0+R+Q-2; anything outside [0,N) is the zero extension
+            long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
+            kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
+            const int r0 = (int)kc + (1 - Q / 2) + seg * R;
 #pragma unroll
-        for (int t = 0; t < NU; ++t) {
-            const int row = r0 + t;
-            u[t] = (row >= 0 && row < N) ? BSL6D_LD(pin + (size_t)row * stride) : 0.0;
+            for (int t = 0; t < NU; ++t) {
+                const int row = r0 + t;
+                u[t] = (row >= 0 && row < N) ? BSL6D_LD(pin + (size_t)row * stride) : 0.0;
+            }
         }
     }
+    if (S > 1) __syncthreads();                            // every segment of a pencil has loaded before any stores
+    if (!live) return;
 
     double w[Q];
     lagrange_weights<Q>(theta, w);
 
 #pragma unroll
-    for (int j = 0; j < N; ++j) {
-        double acc = w[0] * u[PERIODIC ? (j % N) : j];
+    for (int j = 0; j < R; ++j) {
+        double acc = w[0] * u[(PERIODIC && S == 1) ? (j % N) : j];
 #pragma unroll
-        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[PERIODIC ? ((j + m) % N) : (j + m)], acc);
-        BSL6D_ST(pout + (size_t)j * stride, acc);
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[(PERIODIC && S == 1) ? ((j + m) % N) : (j + m)], acc);
+        BSL6D_ST(pout + (size_t)(seg * R + j) * stride, acc);
     }
 }
 

@@ -128,7 +128,7 @@ struct VBlockGeom {
     static constexpr uint32_t SWZ = RB == 128 ? 7u : 3u;   // 16-byte chunk index ^= row bits & SWZ
     static constexpr int PLANE = NV * RB;                  // bytes per j1 plane
     static constexpr int TILE = NV * PLANE;                // bytes per CTA tile
-    static constexpr int T = NV * CW < 256 ? (NV * CW < 32 ? 32 : NV * CW) : 256;   // threads per CTA
+    static constexpr int T = NV * CW < 512 ? (NV * CW < 32 ? 32 : NV * CW) : 512;   // threads per CTA: one per v1/v2 pencil
     static constexpr size_t kSmemBytes = (size_t)TILE + 1024;   // + alignment slack (swizzle pattern repeats at 1 KB)
     static_assert(NV % CL == 0 && (RB == 64 || RB == 128), "tile rows must be 64 or 128 bytes");
     static_assert(PLANE % 1024 == 0 || (RB == 64 && PLANE % 512 == 0), "j1 planes must not disturb the swizzle bits");
@@ -197,35 +197,34 @@ __global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__((VBlockGeom<NV, CL>
             }
         } else {
             // ---- along v3: row piece (j1, j2) x this CTA's CW outputs; inputs from any CTA of the cluster
-            constexpr int RP = (NV * NV + T - 1) / T;      // row pieces per thread
-            double res[RP][CW];
-            if (CL > 1) cooperative_groups::this_cluster().sync();     // the previous sweep's writes, cluster-wide
-#pragma unroll
+            // Hazard: a neighbour reads my boundary columns of row p while I want to overwrite row p.  Rows are
+            // handled in RP rounds (round r = rows r*T .. r*T+T-1 in EVERY CTA of the cluster, each thread one row
+            // piece); within a round everyone reads, the cluster synchronises, everyone writes.  Later rounds touch
+            // other rows, so one barrier per round (plus one up front for the previous sweep's writes) is enough.
+            constexpr int RP = (NV * NV + T - 1) / T;      // rounds
+            if (CL > 1) cooperative_groups::this_cluster().sync();
+#pragma unroll 1
             for (int r = 0; r < RP; ++r) {
                 const uint32_t p = r * T + threadIdx.x;    // row = j1*NV + j2
+                const uint32_t roff = p * RB;
+                const uint32_t sx = ((roff >> 7) & SWZ) << 4;
+                double res[CW];
                 if (p < NV * NV) {
-                    const uint32_t roff = p * RB;
                     const uint32_t rbase = tile + roff;
-                    const uint32_t sx = ((roff >> 7) & SWZ) << 4;
                     const double sval = __ldg(sw.src + src_offset(sw.terms, x * (NV * NV) + p, 0u));
                     vb::window_sweep<NV, CW, Q>(sval, sw.scale, c_lo,
                                                 [&](int col) {
                                                     const uint32_t owner = (uint32_t)col / CW, cl = (uint32_t)col % CW;
                                                     const uint32_t ad = rbase + ((cl * 8) ^ sx);
-                                                    return CL > 1 ? vb::ld_cluster_f64(ad, owner) : vb::lds_f64(ad);
+                                                    if (CL > 1 && owner != rank) return vb::ld_cluster_f64(ad, owner);
+                                                    return vb::lds_f64(ad);
                                                 },
-                                                res[r]);
+                                                res);
                 }
-            }
-            if (CL > 1) cooperative_groups::this_cluster().sync();     // every CTA has read what it needs
-#pragma unroll
-            for (int r = 0; r < RP; ++r) {
-                const uint32_t p = r * T + threadIdx.x;
+                if (CL > 1) cooperative_groups::this_cluster().sync();     // every CTA has read this round's rows
                 if (p < NV * NV) {
-                    const uint32_t roff = p * RB;
-                    const uint32_t sx = ((roff >> 7) & SWZ) << 4;
 #pragma unroll
-                    for (int j = 0; j < CW; ++j) vb::sts_f64(tile + roff + (((uint32_t)j * 8) ^ sx), res[r][j]);
+                    for (int j = 0; j < CW; ++j) vb::sts_f64(tile + roff + (((uint32_t)j * 8) ^ sx), res[j]);
                 }
             }
         }

@@ -62,6 +62,10 @@ def test_v_chain_one_pass_equals_single_sweeps_and_oracle(nv, degree):
     sw = [(d, torch.from_numpy(np.ascontiguousarray(s)).cuda(), m, sc) for d, s, m, sc in sw_host]
     fd = torch.from_numpy(f).cuda()
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        default_passes = ctx.seq_passes(sw)                       # default policy: v3 sweeps stay passes of their own
+        assert 1 < default_passes < len(sw)
+        by_policy = ctx.advect_seq(fd, torch.empty_like(fd), sw)
+        ctx.set_fusion(2)                                         # everything the kernels can do
         assert ctx.seq_passes(sw) == 1                            # nine velocity-space sweeps, one pass
         l0 = ctx.launch_count()
         one = ctx.advect_seq(fd, torch.empty_like(fd), sw)
@@ -71,7 +75,7 @@ def test_v_chain_one_pass_equals_single_sweeps_and_oracle(nv, degree):
         ctx.set_fusion(0)
         assert ctx.seq_passes(sw) == len(sw)
         single = ctx.advect_seq(fd, torch.empty_like(fd), sw)
-    assert torch.equal(one, single) and torch.equal(inplace, single)
+    assert torch.equal(one, single) and torch.equal(inplace, single) and torch.equal(by_policy, single)
     assert rel_err(one, run_oracle(w, f, sw_host)) <= TOL
 
 
@@ -83,6 +87,7 @@ def test_whole_cell_shifts_stay_exact_through_a_v_block_pass():
     one = torch.ones(1, dtype=torch.float64, device="cuda")
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
         sw = [(3, one, 0, 2.0), (4, one, 0, -3.0), (5, one, 0, 9.0), (5, one, 0, -20.0)]   # alpha = -2, +3, -9, +20
+        ctx.set_fusion(2)
         assert ctx.seq_passes(sw) == 1
         out = ctx.advect_seq(fd, torch.empty_like(fd), sw).cpu().numpy()
     ref = f                                                       # shift with zero fill, sweep by sweep
@@ -101,8 +106,9 @@ def test_whole_cell_shifts_stay_exact_through_a_v_block_pass():
 
 
 @pytest.mark.parametrize("pingpong", (False, True))
-def test_strang_step_takes_five_passes_and_matches(pingpong):
-    """x1 | x2,x3 (pair where it pays, else two) | the whole velocity part in ONE pass | x1 | x2,x3."""
+def test_strang_step_passes_and_matches(pingpong):
+    """Fusion mode 2: x1+x2 | x3 | the whole velocity part in ONE pass | x1+x2 | x3 -- five launches.  Default policy:
+    x1 | x2+x3 | v1+v2 | v3 | the three shears | x1 | x2+x3 -- seven.  All of them bit-identical to twelve sweeps."""
     _need_gpu()
     w = wl.C5.reduced((6, 8, 8, 32, 32, 32))
     w = wl.replace(w, degree=7)
@@ -115,30 +121,39 @@ def test_strang_step_takes_five_passes_and_matches(pingpong):
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
         l0 = ctx.launch_count()
         ctx.strang_step(a, tmp, Ed, w.B, w.dt)
-        npass = ctx.launch_count() - l0
-        assert npass <= 7 and npass >= 5, npass
-        ctx.set_fusion(3)                                         # the two-dim tile passes only
-        ctx.strang_step(b.clone(), None, Ed, w.B, w.dt)
+        assert ctx.launch_count() - l0 == 7
+        c5 = b.clone()
+        ctx.set_fusion(2)
+        l0 = ctx.launch_count()
+        ctx.strang_step(c5, tmp, Ed, w.B, w.dt)
+        assert ctx.launch_count() - l0 == 5
+        c3 = b.clone()
+        ctx.set_fusion(3)                                         # round 1's two-dim tile passes only
+        ctx.strang_step(c3, None, Ed, w.B, w.dt)
         ctx.set_fusion(0)
+        l0 = ctx.launch_count()
         ctx.strang_step(b, None, Ed, w.B, w.dt)
-    assert torch.equal(a, b)
+        assert ctx.launch_count() - l0 == 12
+    assert torch.equal(a, b) and torch.equal(c5, b) and torch.equal(c3, b)
     assert rel_err(a, oracle.strang_step(ogrid(w), w.degree, f.copy(), E, w.B, w.dt)) <= TOL
 
 
-def test_oblique_B_rotation_is_one_v_block_pass():
+def test_oblique_B_rotation_in_v_block_passes():
     _need_gpu()
     w = wl.C4.reduced((2, 1, 2, 32, 32, 32))
     f = w.make_f("cpu").numpy()
     B, dt = (0.4, -0.3, 0.6), 0.5
     fd = torch.from_numpy(f).cuda()
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        by_policy = ctx.rotate(fd, torch.empty_like(fd), B, dt)
+        ctx.set_fusion(2)
         l0 = ctx.launch_count()
         out = ctx.rotate(fd, torch.empty_like(fd), B, dt)
         npass = ctx.launch_count() - l0
         ctx.set_fusion(0)
         single = ctx.rotate(fd, torch.empty_like(fd), B, dt)
     assert npass <= 2, npass                                      # 15 shears: two passes of <= 12 sweeps
-    assert torch.equal(out, single)
+    assert torch.equal(out, single) and torch.equal(by_policy, single)
     assert rel_err(out, oracle.rotate(ogrid(w), w.degree, f, B, dt)) <= TOL
 
 
@@ -164,6 +179,7 @@ def test_full_size_C2_v_block_pass_on_sampled_x_points():
     xs[1] = (31, 31, 31)
     before = np.stack([fd[i, j, k].cpu().numpy() for i, j, k in xs])          # [24][32][32][32]
     with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        ctx.set_fusion(2)
         assert ctx.seq_passes(chain) == 1
         ctx.advect_seq(fd, fd, chain)                                          # in place, one launch
     after = np.stack([fd[i, j, k].cpu().numpy() for i, j, k in xs])
