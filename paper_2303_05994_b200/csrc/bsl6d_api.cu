@@ -14,6 +14,7 @@
 #include "fused_api.h"
 #include "fused_kernels.cuh"
 #include "pointwise_kernels.cuh"
+#include "ptile_kernels.cuh"
 #include "sweep_kernels.cuh"
 #include "vblock_kernels.cuh"
 
@@ -36,6 +37,10 @@ struct bsl6d_ctx {
     int field_ready;          // field step: every table and work array is allocated
     int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
+    int fusion_mode;          // as set by bsl6d_set_fusion
+    int use_ptile;            // 1: chains over two dims run as persistent TMA-fed tile passes where a kernel exists
+    int use_fused;            // 1: round-1 two-dim tile kernels (pairs / triples) where no ptile kernel exists
+    int num_sms;
     int vblock_min;           // fewest sweeps a whole-v-block pass is used for
     int use_vblock;           // 1: runs of velocity-space sweeps run as one whole-v-block pass where a kernel exists
     const void* smem_ok[64];  // kernels whose dynamic shared-memory limit has been raised (and to how much)
@@ -66,12 +71,17 @@ struct KernelChoice {
 template <int N, int Q, bool P> constexpr int strided_threads() { return BSL6D_TUNE_T; }
 template <int N, int Q, bool P> constexpr int strided_minblocks() { return BSL6D_TUNE_MINB; }
 #else
+// Pencils that fit 128 registers: 4 blocks of 128 threads (16 warps/SM).  Longer pencils (N = 48 with Q = 10, N = 64)
+// allow only ~12 warps/SM; they run as blocks of 64 threads, 6 (or 4) per SM: the same warps in finer-grained
+// blocks overlap their load / compute / store phases better (C5 x sweeps: 6.19-6.30 -> 6.33-6.58 TB/s in-step).
 template <int N, int Q, bool P>
-constexpr int strided_threads() { return 128; }
+constexpr int strided_regs_wanted() { return 2 * (N + (P ? 0 : Q - 1)) + 2 * Q + 24; }
+template <int N, int Q, bool P>
+constexpr int strided_threads() { return strided_regs_wanted<N, Q, P>() <= 128 ? 128 : 64; }
 template <int N, int Q, bool P>
 constexpr int strided_minblocks() {
-    constexpr int est = 2 * (N + (P ? 0 : Q - 1)) + 2 * Q + 24;      // registers a thread wants
-    return est <= 128 ? 4 : (est <= 176 ? 3 : 2);
+    constexpr int est = strided_regs_wanted<N, Q, P>();
+    return est <= 128 ? 4 : (est <= 176 ? 6 : 4);
 }
 #endif
 
@@ -360,6 +370,9 @@ struct Pass {
     int pattern;
     bool vblock;              // whole-v-block pass (vblock_kernels.cuh)
     bsl6d::VBlockChoice vc;
+    bool ptile;               // persistent TMA-fed two-dim tile pass (ptile_kernels.cuh)
+    bsl6d::PTileChoice pc;
+    int dim_a, dim_b;
 };
 
 bool fused_lookup(int q, int na, int nb, bool pa, bool pb, int pattern, bsl6d::FusedChoice& fc) {
@@ -403,7 +416,50 @@ bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) 
     }
     const size_t blocks = outer * mid * (inner_b / (size_t)fc.C);
     if (blocks > 0x7FFFFFFFull) return false;
-    p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern; p.vblock = false;
+    p.first = i; p.count = cnt; p.fused = true; p.fc = fc; p.pattern = pattern; p.vblock = false; p.ptile = false;
+    return true;
+}
+
+bool ptile_lookup(int q, int na, int nb, bool pa, bool pb, bsl6d::PTileChoice& pc) {
+    switch (q) {
+        case 6: return bsl6d::ptile_lookup_q6(na, nb, pa, pb, pc);
+        case 8: return bsl6d::ptile_lookup_q8(na, nb, pa, pb, pc);
+        case 10: return bsl6d::ptile_lookup_q10(na, nb, pa, pb, pc);
+        default: return false;
+    }
+}
+
+// Can sweeps [i, i+cnt) -- any order of sweeps along exactly two dims a < b, b not the unit-stride dim -- run as one
+// persistent tile pass?
+bool try_ptile(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) {
+    if (cnt < 2 || cnt > bsl6d::kMaxPSweeps) return false;
+    int a = sw[i].dim, b = -1;
+    for (int k = 1; k < cnt; ++k) {
+        const int d = sw[i + k].dim;
+        if (d == a || d == b) continue;
+        if (b >= 0) return false;
+        b = d;
+    }
+    if (b < 0) return false;
+    if (a > b) { const int t = a; a = b; b = t; }
+    const int32_t* n = c->g.n;
+    size_t inner_b = 1, mid = 1, outer = 1;
+    for (int d = b + 1; d < 6; ++d) inner_b *= (size_t)n[d];
+    for (int d = a + 1; d < b; ++d) mid *= (size_t)n[d];
+    for (int d = 0; d < a; ++d) outer *= (size_t)n[d];
+    if (inner_b < (size_t)bsl6d::kPTileC || inner_b % (size_t)bsl6d::kPTileC) return false;
+    if (c->npts > 0xFFFFFFFFull) return false;                        // 32-bit pencil indices in the kernel
+    bsl6d::PTileChoice pc;
+    if (!bsl6d::ptile_available() || !ptile_lookup(c->q, n[a], n[b], a < 3, b < 3, pc)) return false;
+    if (!c->fuse_all) {
+        // same policy as for the round-1 pairs: tiles whose rows lie >= 64 MB apart (x1 on the big grids) do not pay
+        const size_t strideA_bytes = mid * (size_t)n[b] * inner_b * sizeof(double);
+        if (strideA_bytes >= ((size_t)64 << 20)) return false;
+    }
+    const size_t tiles = outer * mid * (inner_b / (size_t)bsl6d::kPTileC);
+    if (tiles > 0x7FFFFFFFull) return false;
+    p.first = i; p.count = cnt; p.fused = false; p.pattern = 0; p.vblock = false; p.ptile = true; p.pc = pc;
+    p.dim_a = a; p.dim_b = b;
     return true;
 }
 
@@ -422,7 +478,7 @@ bool try_vblock(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p
     if (!bsl6d::vblock_lookup(n[3], n[4], n[5], c->q, vc)) return false;
     const size_t nx = (size_t)n[0] * n[1] * n[2];
     if (c->npts > 0xFFFFFFFFull || nx * (size_t)vc.cl > 0x7FFFFFFFull) return false;
-    p.first = i; p.count = cnt; p.fused = false; p.pattern = 0; p.vblock = true; p.vc = vc;
+    p.first = i; p.count = cnt; p.fused = false; p.pattern = 0; p.vblock = true; p.vc = vc; p.ptile = false;
     return true;
 }
 
@@ -439,15 +495,24 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
     // pick[i] > 0: a two-dim tile pass over that many sweeps (or a single sweep); pick[i] < 0: a whole-v-block pass
     // over -pick[i] sweeps.  Ties go to the later candidate: v-block pass > triple > pair > single.
     std::vector<int> best(ns + 1, 0), pick(ns + 1, 1);
-    std::vector<Pass> cand2(ns), cand3(ns), candv(ns);
+    std::vector<Pass> cand2(ns), cand3(ns), candv(ns), candp(ns);
+    std::vector<int> plen(ns, 0);
     for (int i = ns - 1; i >= 0; --i) {
         best[i] = 1 + best[i + 1];
         pick[i] = 1;
-        if (c->fusion && i + 1 < ns && try_fuse(c, sw, i, 2, cand2[i])) {
+        if (c->fusion && c->use_fused && i + 1 < ns && try_fuse(c, sw, i, 2, cand2[i])) {
             if (1 + best[i + 2] < best[i]) { best[i] = 1 + best[i + 2]; pick[i] = 2; }
         }
-        if (c->fusion && i + 2 < ns && try_fuse(c, sw, i, 3, cand3[i])) {
+        if (c->fusion && c->use_fused && i + 2 < ns && try_fuse(c, sw, i, 3, cand3[i])) {
             if (1 + best[i + 3] < best[i]) { best[i] = 1 + best[i + 3]; pick[i] = 3; }
+        }
+        if (c->fusion && c->use_ptile) {
+            // persistent tile passes: ties with the round-1 kernels go to these, longer chains win
+            for (int len = 2; len <= bsl6d::kMaxPSweeps && i + len <= ns; ++len) {
+                Pass p;
+                if (!try_ptile(c, sw, i, len, p)) break;      // a third dim (or the unit-stride dim) ends the chain
+                if (1 + best[i + len] <= best[i]) { best[i] = 1 + best[i + len]; pick[i] = 100 + len; candp[i] = p; }
+            }
         }
         if (c->fusion && c->use_vblock) {
             int run = 0;
@@ -457,15 +522,23 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
             for (int len = c->vblock_min; len <= run; ++len) {
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
-                if (1 + best[i + len] <= best[i]) { best[i] = 1 + best[i + len]; pick[i] = -len; candv[i] = p; }
+                // a whole-v-block pass must save a pass against what the two-dim tiles manage
+                if (1 + best[i + len] < best[i]) { best[i] = 1 + best[i + len]; pick[i] = -len; candv[i] = p; }
             }
         }
     }
-    for (int i = 0; i < ns; i += (pick[i] < 0 ? -pick[i] : pick[i])) {
-        if (pick[i] < 0) passes.push_back(candv[i]);
-        else if (pick[i] == 3) passes.push_back(cand3[i]);
-        else if (pick[i] == 2) passes.push_back(cand2[i]);
-        else passes.push_back(Pass{i, 1, false, {}, 0, false, {}});
+    for (int i = 0; i < ns;) {
+        if (pick[i] < 0) { passes.push_back(candv[i]); i += -pick[i]; }
+        else if (pick[i] >= 100) { passes.push_back(candp[i]); i += pick[i] - 100; }
+        else if (pick[i] == 3) { passes.push_back(cand3[i]); i += 3; }
+        else if (pick[i] == 2) { passes.push_back(cand2[i]); i += 2; }
+        else {
+            Pass p;
+            std::memset(&p, 0, sizeof(p));
+            p.first = i; p.count = 1;
+            passes.push_back(p);
+            i += 1;
+        }
     }
     return BSL6D_OK;
 }
@@ -528,7 +601,40 @@ int launch_vblock(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDe
     return BSL6D_OK;
 }
 
+int launch_ptile(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDesc* sw, const Pass& p,
+                 cudaStream_t stream) {
+    const int a = p.dim_a, b = p.dim_b;
+    const int32_t* n = c->g.n;
+    size_t inner_b = 1, mid = 1, outer = 1;
+    for (int d = b + 1; d < 6; ++d) inner_b *= (size_t)n[d];
+    for (int d = a + 1; d < b; ++d) mid *= (size_t)n[d];
+    for (int d = 0; d < a; ++d) outer *= (size_t)n[d];
+    bsl6d::PTileArgs pa;
+    std::memset(&pa, 0, sizeof(pa));
+    pa.nsweeps = (uint32_t)p.count;
+    pa.mid = (uint32_t)mid;
+    pa.inner_b = (uint32_t)inner_b;
+    pa.nchunks = (uint32_t)(inner_b / (size_t)bsl6d::kPTileC);
+    pa.ntiles = (uint32_t)(outer * mid * (size_t)pa.nchunks);
+    for (int k = 0; k < p.count; ++k) {
+        const SweepDesc& s = sw[p.first + k];
+        pa.sw[k].src = s.src;
+        pa.sw[k].scale = s.scale;
+        pa.sw[k].along_b = s.dim == b ? 1 : 0;
+        int rc = build_src_terms(n, s.dim, s.mask, pa.sw[k].terms);
+        if (rc) return rc;
+    }
+    if (int rcs = allow_smem(c, p.pc.fn, p.pc.smem)) return rcs;
+    cudaError_t e = bsl6d::ptile_launch(p.pc, f_in, f_out, outer, mid, inner_b, pa, c->num_sms, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
+}
+
 int launch_pass(bsl6d_ctx* c, const double* src, double* dst, const SweepDesc* sw, const Pass& p, cudaStream_t st) {
+    if (p.ptile) return launch_ptile(c, src, dst, sw, p, st);
     if (p.vblock) return launch_vblock(c, src, dst, sw, p, st);
     if (p.fused) return launch_fused(c, src, dst, sw, p, st);
     const SweepDesc& s = sw[p.first];
@@ -761,7 +867,18 @@ int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
     c->fusion = 1;
     c->fuse_all = 0;
     c->use_vblock = 1;
+    c->use_ptile = 1;
+    c->use_fused = 1;
+    c->fusion_mode = 1;
     c->vblock_min = 2;
+    {
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+            (void)cudaGetLastError();
+            sms = 148;
+        }
+        c->num_sms = sms;
+    }
 
     std::vector<double> nodes(nn);
     size_t off = 0;
@@ -914,11 +1031,14 @@ int bsl6d_seq_passes(bsl6d_ctx* c, const bsl6d_sweep* sweeps, int nsweeps) {
 
 int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     if (!c) return BSL6D_EINVAL;
-    if (enable < 0 || enable > 3) return BSL6D_EINVAL;
-    const int old = !c->fusion ? 0 : (c->fuse_all ? 2 : (c->use_vblock ? 1 : 3));
+    if (enable < 0 || enable > 4) return BSL6D_EINVAL;
+    const int old = c->fusion_mode;
+    c->fusion_mode = enable;
     c->fusion = enable ? 1 : 0;
     c->fuse_all = enable == 2 ? 1 : 0;
+    c->use_ptile = (enable == 1 || enable == 2) ? 1 : 0;      // 3: round-1 tile kernels only; 4: those + v-block passes
     c->use_vblock = enable == 3 ? 0 : 1;
+    c->use_fused = 1;
     return old;
 }
 

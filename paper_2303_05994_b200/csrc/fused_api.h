@@ -39,6 +39,23 @@ cudaError_t vblock_launch(const VBlockChoice& vc, const double* f_in, double* f_
                           const VBlockArgs& args, cudaStream_t stream);
 }  // namespace bsl6d
 
+// ---- persistent TMA-fed two-dim tile passes (ptile_kernels.cuh, bsl6d_ptile.cu) -----------------------------------
+namespace bsl6d {
+struct PTileArgs;
+struct PTileChoice {
+    const void* fn;        // __global__ void (*)(CUtensorMap, CUtensorMap, PTileArgs)
+    int threads;
+    size_t smem;
+    int na, nb;
+};
+bool ptile_lookup_q6(int na, int nb, bool pa, bool pb, PTileChoice& out);
+bool ptile_lookup_q8(int na, int nb, bool pa, bool pb, PTileChoice& out);
+bool ptile_lookup_q10(int na, int nb, bool pa, bool pb, PTileChoice& out);
+bool ptile_available();    // is cuTensorMapEncodeTiled reachable through the runtime?
+cudaError_t ptile_launch(const PTileChoice& pc, const double* f_in, double* f_out, uint64_t outer, uint64_t mid,
+                         uint64_t inner_b, const PTileArgs& args, int num_sms, cudaStream_t stream);
+}  // namespace bsl6d
+
 // ---- pointwise (odd q, per-point displacement) kernels, bsl6d_pointwise.cu -------------------------------------
 namespace bsl6d {
 struct PointwiseChoice {
