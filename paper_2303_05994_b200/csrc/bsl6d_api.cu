@@ -452,9 +452,12 @@ bool try_ptile(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p)
     bsl6d::PTileChoice pc;
     if (!bsl6d::ptile_available() || !ptile_lookup(c->q, n[a], n[b], a < 3, b < 3, pc)) return false;
     if (!c->fuse_all) {
-        // same policy as for the round-1 pairs: tiles whose rows lie >= 64 MB apart (x1 on the big grids) do not pay
-        const size_t strideA_bytes = mid * (size_t)n[b] * inner_b * sizeof(double);
-        if (strideA_bytes >= ((size_t)64 << 20)) return false;
+        // Policy from measurement: one TMA box per tile keeps 64 KB in flight per SM, which is
+        // enough when the 64-byte rows of a tile lie close together (v1+v2: 256 B apart; x3+v1: 8 KB) and not when every
+        // row sits in its own DRAM page (x2+x3: 256 KB apart -- there the round-1 kernels, which keep 2 x 64 KB of
+        // register-staged loads in flight, are faster).
+        const size_t strideB_bytes = inner_b * sizeof(double);
+        if (strideB_bytes > ((size_t)64 << 10)) return false;
     }
     const size_t tiles = outer * mid * (inner_b / (size_t)bsl6d::kPTileC);
     if (tiles > 0x7FFFFFFFull) return false;
@@ -522,8 +525,10 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
             for (int len = c->vblock_min; len <= run; ++len) {
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
-                // a whole-v-block pass must save a pass against what the two-dim tiles manage
-                if (1 + best[i + len] < best[i]) { best[i] = 1 + best[i + len]; pick[i] = -len; candv[i] = p; }
+                // Measured: for three or more sweeps the v-block kernel (two CTAs per SM, swizzled
+                // tile) is at least as fast as the persistent tile pass, for a pair the persistent pass wins.
+                const int total = 1 + best[i + len];
+                if (total < best[i] || (total == best[i] && len >= 3)) { best[i] = total; pick[i] = -len; candv[i] = p; }
             }
         }
     }
