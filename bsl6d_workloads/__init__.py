@@ -185,7 +185,11 @@ C5 = _mk("C5", (48, 48, 48, 32, 32, 32), FOUR_PI, 6.0, degree=9, dt=0.05, seed=1
 #: per-point displacements alpha/dx in [-1, 1] (see random_shifts).  degree here is only the default even-q context.
 P37 = _mk("P37", (37,) * 6, FOUR_PI, 6.0, degree=7, dt=0.05, seed=1037, noise_amp=1e-3, kind="maxwell_x1")
 
-CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5, P37)}
+#: An extent without specialised sweep kernels (36 is not in {8,16,32,37,48,64}): every sweep of this workload runs the
+#: run-time-extent fallback kernels, so that their throughput can be timed and profiled (bench.py --workload G36).
+G36 = _mk("G36", (36,) * 6, FOUR_PI, 6.0, degree=7, dt=0.05, seed=1036, noise_amp=1e-3, kind="maxwell_x1")
+
+CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5, P37, G36)}
 
 
 def random_shifts(shape: Sequence[int], seed: int, device="cpu", whole_cells: bool = False,

@@ -72,16 +72,22 @@ template <int N, int Q, bool P> constexpr int strided_threads() { return BSL6D_T
 template <int N, int Q, bool P> constexpr int strided_minblocks() { return BSL6D_TUNE_MINB; }
 #else
 // Pencils that fit 128 registers: 4 blocks of 128 threads (16 warps/SM).  Longer pencils (N = 48 with Q = 10, N = 64)
-// allow only ~12 warps/SM; they run as blocks of 64 threads, 6 (or 4) per SM: the same warps in finer-grained
-// blocks overlap their load / compute / store phases better (C5 x sweeps: 6.19-6.30 -> 6.33-6.58 TB/s in-step).
+// allow only ~12 warps/SM; they run as blocks of 64 threads, 6 (or 4) per SM.  Measured against 3 blocks of 128
+// threads in alternating runs on one box: no difference beyond noise (C5 x sweeps 6.21-6.48 TB/s either way) -- inside a
+// long step these kernels are held back by the 1 kW power cap (SM clock ~1.55 GHz), not by the block shape.  Two or
+// four threads per pencil (S > 1 below) were slower (6.09 / 5.0-5.6 TB/s): the shared rows are re-read through L1/L2.
 template <int N, int Q, bool P>
 constexpr int strided_regs_wanted() { return 2 * (N + (P ? 0 : Q - 1)) + 2 * Q + 24; }
+#ifndef BSL6D_TUNE_LONG_T
+#define BSL6D_TUNE_LONG_T 64
+#define BSL6D_TUNE_LONG_MINB 6
+#endif
 template <int N, int Q, bool P>
-constexpr int strided_threads() { return strided_regs_wanted<N, Q, P>() <= 128 ? 128 : 64; }
+constexpr int strided_threads() { return strided_regs_wanted<N, Q, P>() <= 128 ? 128 : BSL6D_TUNE_LONG_T; }
 template <int N, int Q, bool P>
 constexpr int strided_minblocks() {
     constexpr int est = strided_regs_wanted<N, Q, P>();
-    return est <= 128 ? 4 : (est <= 176 ? 6 : 4);
+    return est <= 128 ? 4 : (est <= 176 ? BSL6D_TUNE_LONG_MINB : (BSL6D_TUNE_LONG_MINB * 2) / 3);
 }
 #endif
 
@@ -119,7 +125,7 @@ KernelChoice unit_choice() {
     constexpr int S = unit_segments<N, Q>();
     constexpr int T = unit_threads<N, Q>();
     constexpr int MINB = unit_minblocks<N, Q>();
-    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N + 1), 1, S};
+    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N | 1), 1, S};
 }
 
 template <int N, bool P>
@@ -139,6 +145,7 @@ bool strided_lookup(int n, int q, KernelChoice& c) {
         case 8: return strided_by_q<8, P>(q, c);
         case 16: return strided_by_q<16, P>(q, c);
         case 32: return strided_by_q<32, P>(q, c);
+        case 37: return strided_by_q<37, P>(q, c);          // the paper's benchmark extent
         case 48: return strided_by_q<48, P>(q, c);
         case 64: return strided_by_q<64, P>(q, c);
         default: return false;
@@ -161,6 +168,7 @@ bool unit_lookup(int n, int q, KernelChoice& c) {
         case 8: return unit_by_q<8>(q, c);
         case 16: return unit_by_q<16>(q, c);
         case 32: return unit_by_q<32>(q, c);
+        case 37: return unit_by_q<37>(q, c);
         case 48: return unit_by_q<48>(q, c);
         case 64: return unit_by_q<64>(q, c);
         default: return false;
@@ -327,13 +335,20 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     } else {
         // strided: kc.gen_T = segments per pencil (threads / segments pencils per block); generic: gen_T = threads
         const uint64_t pencils = kc.kind == 0 ? (uint64_t)kc.threads / (uint64_t)kc.gen_T : (uint64_t)kc.threads;
-        const uint64_t lim = inner < pencils ? inner : pencils;
-        a.ti_log2 = ceil_pow2_log2(lim);
-        const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)pencils / TI;
-        a.nib = (uint32_t)((inner + TI - 1) / TI);
-        const uint64_t nbo = (outer + TO - 1) / TO;
-        if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
-        grid = (unsigned)((uint64_t)a.nib * nbo);
+        if (kc.kind == 0 && kc.gen_T == 1 && inner % 32 != 0 && inner > 1) {
+            // odd inner extents (37^k): flattened pencil index, every lane busy
+            a.ti_log2 = bsl6d::kFlatPencils;
+            a.nib = (uint32_t)(inner * outer);
+            grid = (unsigned)((inner * outer + pencils - 1) / pencils);
+        } else {
+            const uint64_t lim = inner < pencils ? inner : pencils;
+            a.ti_log2 = ceil_pow2_log2(lim);
+            const uint32_t TI = 1u << a.ti_log2, TO = (uint32_t)pencils / TI;
+            a.nib = (uint32_t)((inner + TI - 1) / TI);
+            const uint64_t nbo = (outer + TO - 1) / TO;
+            if ((uint64_t)a.nib * nbo > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
+            grid = (unsigned)((uint64_t)a.nib * nbo);
+        }
     }
 
     cudaError_t e;

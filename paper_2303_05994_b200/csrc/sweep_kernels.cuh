@@ -32,6 +32,7 @@
 namespace bsl6d {
 
 constexpr int kMaxSrcTerms = 5;
+constexpr uint32_t kFlatPencils = 31;                      // SweepArgs::ti_log2 value selecting flattened pencil indexing
 
 // Where a pencil finds its shift source: the array seen along the swept dim is [outer][N][inner]; the source is a
 // dense C-order array over a subset of the other dims, so its index is a sum of up to five
@@ -53,7 +54,7 @@ struct SweepArgs {
     uint32_t outer;        // product of extents of dims slower than the swept one
     uint32_t n;            // extent of the swept dim (== template N in the specialised kernels)
     uint32_t ti_log2;      // strided: threads of a block along `inner` = 1 << ti_log2
-    uint32_t nib;          // strided: number of inner chunks (= ceil(inner / TI))
+    uint32_t nib;          // strided: number of inner chunks (= ceil(inner / TI)); flattened mode: number of pencils
     SrcTerms terms;
 };
 
@@ -129,12 +130,23 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
     constexpr int R = N / S;                               // outputs per thread
     const uint32_t tp = S == 1 ? threadIdx.x : threadIdx.x % TP;
     const int seg = S == 1 ? 0 : (int)(threadIdx.x / TP);
-    const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
-    const uint32_t bo = blockIdx.x / a.nib;
-    const uint32_t bi = blockIdx.x - bo * a.nib;
-    const uint32_t i = (bi << a.ti_log2) + (tp & ti_mask);
-    const uint32_t o = bo * (TP >> a.ti_log2) + (tp >> a.ti_log2);
-    const bool live = i < a.inner && o < a.outer;
+    uint32_t i, o;
+    bool live;
+    if (a.ti_log2 == kFlatPencils) {
+        // `inner` is not a multiple of the warp width (37^k): lanes run along the flattened pencil index so that
+        // every lane has work; a warp then covers the tail of one row segment and the head of the next
+        const uint32_t p = blockIdx.x * TP + tp;
+        live = p < a.nib;                                   // nib = number of pencils in this mode
+        o = p / a.inner;
+        i = p - o * a.inner;
+    } else {
+        const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
+        const uint32_t bo = blockIdx.x / a.nib;
+        const uint32_t bi = blockIdx.x - bo * a.nib;
+        i = (bi << a.ti_log2) + (tp & ti_mask);
+        o = bo * (TP >> a.ti_log2) + (tp >> a.ti_log2);
+        live = i < a.inner && o < a.outer;
+    }
     if (S == 1 && !live) return;
 
     long long k = 0;
@@ -197,8 +209,8 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
 template <int N, int Q, int S, int T, int MINB>
 __global__ void __launch_bounds__(T, MINB) sweep_unit_kernel(const SweepArgs a) {
     static_assert(N % S == 0 && T % (32 * S) == 0, "segments must tile the pencil and the block");
-    extern __shared__ double tile[];                       // PB * (N+1)
-    constexpr int LD = N + 1;
+    extern __shared__ double tile[];                       // PB * LD
+    constexpr int LD = N | 1;                              // odd row pitch: "lane = pencil" accesses are conflict-free
     constexpr int PB = T / S;                              // pencils per block
     constexpr int R = N / S;                               // outputs per thread
     constexpr int NE = PB * N;                             // elements per full block

@@ -116,8 +116,10 @@ GRIDS = [
     ((5, 3, 9, 1, 1, 1), 3),          # degenerate: x3 is periodic AND unit-stride (inner == 1) -> strided fallback
     ((1, 1, 1, 7, 5, 11), 5),         # no x extent at all
     ((13, 1, 1, 21, 1, 1), 1),        # 1D1V, linear interpolation (q = 2)
-    ((2, 1, 37, 1, 1, 40), 7),        # the paper's extent 37 (fallback for even q) + unit-stride fallback
-    ((37, 2, 2, 37, 2, 37), 7),       # 37 in strided periodic, strided zero and unit-stride position
+    ((2, 1, 37, 1, 1, 40), 7),        # the paper's extent 37 (periodic, inner = 40) + unit-stride fallback (40)
+    ((37, 2, 2, 37, 2, 37), 7),       # strided<37,8> periodic + zero with flattened pencil indexing, unit<37,8>
+    ((3, 37, 37, 37, 37, 37), 9),     # strided<37,10> on inner extents 37^k (no multiple of the warp width), unit<37,10>
+    ((36, 3, 2, 36, 2, 36), 5),       # extent 36: no specialised instance -> generic strided + generic unit, q = 6
 ]
 
 
