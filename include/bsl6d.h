@@ -128,6 +128,24 @@ BSL6D_API int bsl6d_advect_seq(bsl6d_ctx* ctx, const double* f_in, double* f_out
 BSL6D_API int bsl6d_seq_passes(bsl6d_ctx* ctx, const bsl6d_sweep* sweeps, int nsweeps);
 BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
 
+/* ---- slab decomposition along x1 (section 3.3, 323) --------------------
+ * The paper distributes f over MPI ranks and gives every rank halo cells around its sub-domain:
+ * the interpolation along a distributed dim then reads the neighbour's points from the halo instead of wrapping.
+ * Here the slowest dim x1 is the one to distribute (each rank then owns one contiguous slab, and every sweep but
+ * the x1 sweep, the rotation and the density moment stay local).  A rank keeps its L = n0/R planes plus w halo planes
+ * on either side in ONE array of (L + 2w) x n1 x ... x n5 doubles and uses two contexts on it:
+ *   - a context for the grid (L, n1, .., n5) on the interior pointer f + w*n1*..*n5: all sweeps along dims 1-5,
+ *     bsl6d_rotate, bsl6d_density (x2, x3 stay periodic, they are not distributed);
+ *   - a context for the grid (L + 2w, n1, .., n5) with bsl6d_set_boundary(ctx, 0, 1): the x1 sweep over the whole
+ *     array.  Dim 0 is then zero-extended instead of periodic, and with w >= q/2 + max|displacement in cells| no
+ *     interior output ever reads beyond the halo; halo outputs are meaningless and are overwritten by the next
+ *     exchange.  The interior outputs are bit-identical to those of the periodic sweep on the undivided grid.
+ * The halo exchange itself (the neighbour's w boundary planes, contiguous: one copy or one send/recv per side) is
+ * plumbing and lives in the Python layer (torch.distributed over NCCL); see paper_2303_05994_b200/slab.py.
+ * open = 1 opens dim 0, 1 or 2; open = 0 makes it periodic again.  Returns the old setting or BSL6D_EINVAL.
+ * bsl6d_field_* and bsl6d_vp_step need a fully periodic x grid and return BSL6D_EUNSUPPORTED on an opened context. */
+BSL6D_API int bsl6d_set_boundary(bsl6d_ctx* ctx, int dim, int open);
+
 /* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);

@@ -20,7 +20,7 @@ SYMBOLS = (
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
-    "bsl6d_advect_pointwise",
+    "bsl6d_advect_pointwise", "bsl6d_set_boundary",
 )
 
 OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
@@ -80,6 +80,7 @@ def load_library() -> C.CDLL:
     lib.bsl6d_advect_seq.argtypes = [vp, dp, dp, C.POINTER(Sweep), C.c_int, vp]
     lib.bsl6d_seq_passes.argtypes = [vp, C.POINTER(Sweep), C.c_int]
     lib.bsl6d_set_fusion.argtypes = [vp, C.c_int]
+    lib.bsl6d_set_boundary.argtypes = [vp, C.c_int, C.c_int]
     lib.bsl6d_advect_pointwise.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, vp]
     lib.bsl6d_field_poisson.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
     lib.bsl6d_field_adiabatic.argtypes = [vp, dp, C.c_double, C.c_double, C.POINTER(C.c_void_p), vp]
@@ -240,6 +241,13 @@ class Context:
         rc = self._lib.bsl6d_set_fusion(self._h, int(mode))
         if rc < 0:
             self._check(rc, "bsl6d_set_fusion")
+        return rc
+
+    def set_boundary(self, dim: int, open_: bool) -> int:
+        """Open (zero-extend) or close (periodic) x dim `dim`; returns the old setting (slab decomposition)."""
+        rc = self._lib.bsl6d_set_boundary(self._h, int(dim), 1 if open_ else 0)
+        if rc < 0:
+            self._check(rc, "bsl6d_set_boundary")
         return rc
 
     def advect_pointwise(self, f_in, f_out, dim: int, alpha_cells, q: int, stream=None):

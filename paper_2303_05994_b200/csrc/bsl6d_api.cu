@@ -37,6 +37,7 @@ struct bsl6d_ctx {
     int field_ready;          // field step: every table and work array is allocated
     int fuse_all;             // tuning/testing: ignore the pay-off policy and fuse wherever a kernel exists
     int fusion;               // 1: consecutive sweeps over two dims run as one fused pass where a kernel exists
+    int open_x[3];            // 1: this x dim is NOT periodic but zero-extended (a slab with halo planes)
     int fusion_mode;          // as set by bsl6d_set_fusion
     int use_ptile;            // 1: chains over two dims run as persistent TMA-fed tile passes where a kernel exists
     int use_fused;            // 1: round-1 two-dim tile kernels (pairs / triples) where no ptile kernel exists
@@ -54,6 +55,9 @@ struct bsl6d_ctx {
 };
 
 namespace {
+
+// dims 0-2 are periodic unless bsl6d_set_boundary opened them (slab decomposition); dims 3-5 are zero-extended
+bool is_periodic(const bsl6d_ctx* c, int dim) { return dim < 3 && !c->open_x[dim]; }
 
 typedef void (*sweep_fn)(const SweepArgs);
 
@@ -206,7 +210,7 @@ const void* generic_unit_fn(int q, int T) { return T == 64 ? generic_unit_by_q<6
 // Which kernel serves a sweep along `dim`?  (Also used by bsl6d_kernel_name.)
 int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     const int n = c->g.n[dim];
-    const bool periodic = dim < 3;
+    const bool periodic = is_periodic(c, dim);
     size_t inner = 1;
     for (int d = dim + 1; d < 6; ++d) inner *= (size_t)c->g.n[d];
     bool ok;
@@ -357,7 +361,7 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
         if (!gfn) return BSL6D_EUNSUPPORTED;
         rc = allow_smem(c, gfn, kc.smem);
         if (rc) return rc;
-        int per = dim < 3 ? 1 : 0;
+        int per = is_periodic(c, dim) ? 1 : 0;
         void* gargs[] = {(void*)&a, (void*)&per};                  // the unit-stride kernel takes only `a`
         grid = (unsigned)((inner * outer + (size_t)kc.gen_T - 1) / (size_t)kc.gen_T);
         e = cudaLaunchKernel(gfn, dim3(grid), dim3(kc.gen_T), gargs, kc.smem, stream);
@@ -420,7 +424,7 @@ bool try_fuse(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p) 
     if (inner_b < 2) return false;
     const int pattern = cnt == 2 ? bsl6d::kPatAB : bsl6d::kPatABA;
     bsl6d::FusedChoice fc;
-    if (!fused_lookup(c->q, n[a], n[b], a < 3, b < 3, pattern, fc)) return false;
+    if (!fused_lookup(c->q, n[a], n[b], is_periodic(c, a), is_periodic(c, b), pattern, fc)) return false;
     if (inner_b % (size_t)fc.C) return false;
     if (c->npts > 0xFFFFFFFFull) return false;                        // 32-bit pencil indices in the kernel
     // Policy from measurement: a pair only pays with >= 64-byte row segments and a tile whose
@@ -465,7 +469,7 @@ bool try_ptile(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p)
     if (inner_b < (size_t)bsl6d::kPTileC || inner_b % (size_t)bsl6d::kPTileC) return false;
     if (c->npts > 0xFFFFFFFFull) return false;                        // 32-bit pencil indices in the kernel
     bsl6d::PTileChoice pc;
-    if (!bsl6d::ptile_available() || !ptile_lookup(c->q, n[a], n[b], a < 3, b < 3, pc)) return false;
+    if (!bsl6d::ptile_available() || !ptile_lookup(c->q, n[a], n[b], is_periodic(c, a), is_periodic(c, b), pc)) return false;
     if (!c->fuse_all) {
         // Policy from measurement: one TMA box per tile keeps 64 KB in flight per SM, which is
         // enough when the 64-byte rows of a tile lie close together (v1+v2: 256 B apart; x3+v1: 8 KB) and not when every
@@ -809,6 +813,7 @@ int field_solve(bsl6d_ctx* c, const double* rho, int adiabatic, double c1, doubl
                 cudaStream_t st) {
     if (!c || !rho || !E || !E[0] || !E[1] || !E[2]) return BSL6D_EINVAL;
     if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
+    if (c->open_x[0] || c->open_x[1] || c->open_x[2]) return BSL6D_EUNSUPPORTED;   // spectral solve: periodic x only
     int rc = check_device(c);
     if (rc) return rc;
     rc = field_setup(c);
@@ -959,10 +964,10 @@ int bsl6d_kernel_name(const bsl6d_ctx* c, int dim, char* buf, int buflen) {
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q, k.gen_T, k.threads);
     else if (k.kind == 0 && k.gen_T > 1)
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q,
-                      dim < 3 ? "periodic" : "zero", k.gen_T, k.threads);
+                      is_periodic(c, dim) ? "periodic" : "zero", k.gen_T, k.threads);
     else
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
-                      dim < 3 ? "periodic" : "zero", k.threads);
+                      is_periodic(c, dim) ? "periodic" : "zero", k.threads);
     return BSL6D_OK;
 }
 
@@ -1049,6 +1054,13 @@ int bsl6d_seq_passes(bsl6d_ctx* c, const bsl6d_sweep* sweeps, int nsweeps) {
     return rc ? rc : (int)passes.size();
 }
 
+int bsl6d_set_boundary(bsl6d_ctx* c, int dim, int open) {
+    if (!c || dim < 0 || dim > 2 || (open != 0 && open != 1)) return BSL6D_EINVAL;
+    const int old = c->open_x[dim];
+    c->open_x[dim] = open;
+    return old;
+}
+
 int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     if (!c) return BSL6D_EINVAL;
     if (enable < 0 || enable > 4) return BSL6D_EINVAL;
@@ -1075,7 +1087,7 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
     for (int d = 0; d < dim; ++d) outer *= (size_t)n[d];
     if (inner * outer > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
     bsl6d::PointwiseChoice pc;
-    if (!bsl6d::pointwise_lookup(n[dim], q, dim < 3, inner == 1, pc)) return BSL6D_EUNSUPPORTED;
+    if (!bsl6d::pointwise_lookup(n[dim], q, is_periodic(c, dim), inner == 1, pc)) return BSL6D_EUNSUPPORTED;
     bsl6d::PointwiseArgs a;
     std::memset(&a, 0, sizeof(a));
     a.in = f_in;
@@ -1085,7 +1097,7 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
     a.outer = (uint32_t)outer;
     unsigned grid;
     if (pc.unit) {
-        grid = (unsigned)((outer + (size_t)pc.threads - 1) / (size_t)pc.threads);
+        grid = (unsigned)((outer + (size_t)pc.unit - 1) / (size_t)pc.unit);
     } else {
         a.npencil = (uint32_t)(inner * outer);
         grid = (unsigned)((inner * outer + (size_t)pc.threads - 1) / (size_t)pc.threads);

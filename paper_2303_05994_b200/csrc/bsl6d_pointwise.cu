@@ -16,7 +16,13 @@ bool by_kind(bool periodic, bool unit, PointwiseChoice& c) {
     constexpr int T = 128;
     if (unit) {
         if (periodic) return false;
-        c = PointwiseChoice{(const void*)pointwise_unit_kernel<N, Q, T, 2>, T, 2 * sizeof(double) * T * (N + 1), 1};
+        constexpr int S = N >= 16 ? 4 : 1, PB = 64;        // 64 pencils x 4 segments per block
+        constexpr size_t smem = 2 * sizeof(double) * PB * (N | 1);
+#ifndef BSL6D_TUNE_PWMINB
+#define BSL6D_TUNE_PWMINB 3
+#endif
+        constexpr int MINB = S == 1 ? 8 : BSL6D_TUNE_PWMINB;   // the weight evaluation wants ~85 registers
+        c = PointwiseChoice{(const void*)pointwise_unit_kernel<N, Q, S, PB, MINB>, PB * S, smem, PB};
     } else if (periodic) {
         c = PointwiseChoice{(const void*)pointwise_strided_kernel<N, Q, true, T, pw_minblocks<N, Q>()>, T, 0, 0};
     } else {

@@ -62,7 +62,7 @@ struct PointwiseChoice {
     const void* fn;        // __global__ void (*)(PointwiseArgs)
     int threads;
     size_t smem;
-    int unit;              // 1: unit-stride kernel (block = `threads` pencils)
+    int unit;              // > 0: unit-stride kernel, a block takes this many pencils
 };
 bool pointwise_lookup(int n, int q, bool periodic, bool unit_stride, PointwiseChoice& out);
 }  // namespace bsl6d

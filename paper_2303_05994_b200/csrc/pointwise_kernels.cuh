@@ -106,49 +106,68 @@ __global__ void __launch_bounds__(T, MINB) pointwise_strided_kernel(const Pointw
     }
 }
 
-// unit-stride dim (inner == 1, always a v dim): T pencils per block, f and alpha transposed through two padded
-// shared-memory tiles; results overwrite the alpha tile (alpha_j is consumed when out_j is produced).
-template <int N, int Q, int T, int MINB>
-__global__ void __launch_bounds__(T, MINB) pointwise_unit_kernel(const PointwiseArgs a) {
-    extern __shared__ double tiles[];                      // 2 x T x (N+1)
-    constexpr int LD = N + 1;
+// unit-stride dim (inner == 1, always a v dim): PB pencils per block, f and alpha transposed through two padded
+// shared-memory tiles (odd row pitch: "lane = pencil" accesses are conflict-free); results overwrite the alpha tile
+// (alpha_j is consumed by the one thread that produces out_j).  A pencil is cut into S segments of R = ceil(N/S)
+// outputs, one thread each (the lanes of a warp share the segment): a thread then holds R+Q-1 values instead of N and
+// evaluates R weight sets instead of N, so that a block has S times the warps for the same tile -- the one-thread-
+// per-pencil version of round 1 ran 8 warps per SM (3.5-4.5 TB/s at 37^6).
+template <int N, int Q, int S, int PB, int MINB>
+__global__ void __launch_bounds__(PB * S, MINB) pointwise_unit_kernel(const PointwiseArgs a) {
+    extern __shared__ double tiles[];                      // 2 x PB x LD
+    constexpr int T = PB * S;
+    constexpr int LD = N | 1;
+    constexpr int H = (Q - 1) / 2;
+    constexpr int R = (N + S - 1) / S;
     double* tf = tiles;
-    double* ta = tiles + T * LD;
-    const size_t p0 = (size_t)blockIdx.x * T;
-    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    double* ta = tiles + PB * LD;
+    const size_t p0 = (size_t)blockIdx.x * PB;
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)PB ? ((size_t)a.outer - p0) : (size_t)PB);
     const uint32_t nelem = np * N;
     const double* pin = a.in + p0 * N;
     const double* pal = a.alpha + p0 * N;
     double* pout = a.out + p0 * N;
+#pragma unroll 4
+    for (uint32_t e = threadIdx.x; e < nelem; e += T) {
+        const uint32_t s = (e / N) * LD + (e % N);
+        tf[s] = __ldcs(pin + e);
+        ta[s] = __ldcs(pal + e);
+    }
+    __syncthreads();
+    const uint32_t pl = threadIdx.x % PB;
+    const int j0 = (int)(threadIdx.x / PB) * R;
+    if (pl < np) {
+        const double* rowf = tf + pl * LD;
+        double* rowa = ta + pl * LD;
+        double u[R + Q - 1];                               // u[t] = f[j0 - H + t], zero outside the pencil
 #pragma unroll
-    for (int it = 0; it < N; ++it) {
-        const uint32_t e = it * T + threadIdx.x;
-        if (e < nelem) {
-            const uint32_t s = (e / N) * LD + (e % N);
-            tf[s] = __ldcs(pin + e);
-            ta[s] = __ldcs(pal + e);
+        for (int t = 0; t < R + Q - 1; ++t) {
+            const int c = j0 - H + t;
+            u[t] = (c >= 0 && c < N) ? rowf[c] : 0.0;
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = j0 + r;
+            if (j < N) {
+                double w[Q];
+                lagrange_weights_odd<Q>(rowa[j], w);
+                // the terms of stencil_at<N, Q, false> in the same order; a node outside the pencil contributes nothing
+                double acc = 0.0;
+                bool first = true;
+#pragma unroll
+                for (int m = 0; m < Q; ++m) {
+                    const int jj = j + m - H;
+                    if (jj < 0 || jj >= N) continue;
+                    acc = first ? w[m] * u[r + m] : fma(w[m], u[r + m], acc);
+                    first = false;
+                }
+                rowa[j] = acc;
+            }
         }
     }
     __syncthreads();
-    if (threadIdx.x < np) {
-        const double* rowf = tf + threadIdx.x * LD;
-        double* rowa = ta + threadIdx.x * LD;
-        double u[N];
-#pragma unroll
-        for (int t = 0; t < N; ++t) u[t] = rowf[t];
-#pragma unroll
-        for (int j = 0; j < N; ++j) {
-            double w[Q];
-            lagrange_weights_odd<Q>(rowa[j], w);
-            rowa[j] = stencil_at<N, Q, false>(u, w, j);
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int it = 0; it < N; ++it) {
-        const uint32_t e = it * T + threadIdx.x;
-        if (e < nelem) __stcs(pout + e, ta[(e / N) * LD + (e % N)]);
-    }
+#pragma unroll 4
+    for (uint32_t e = threadIdx.x; e < nelem; e += T) __stcs(pout + e, ta[(e / N) * LD + (e % N)]);
 }
 
 }  // namespace bsl6d

@@ -1,0 +1,220 @@
+"""x1-slab decomposition with halo exchange (section 3.3, 323, 349 eq (9)).
+
+The paper distributes f over MPI ranks and surrounds every sub-domain with halo cells; the
+1-D interpolation along a distributed dim reads its neighbour's points from the halo, exchanged point-to-point
+before the sweep.  On a B200 node the natural cut is along x1, the slowest dim of the C-order layout:
+each rank owns one contiguous slab of L = n0/R planes, every sweep along x2..v3, the rotation and the density moment
+rho(x) are local (no all-reduce: a rank owns whole v-blocks), and only the x1 sweep needs the neighbours'
+w = q/2 + ceil(max |displacement in cells|) boundary planes -- contiguous blocks of w*n1*n2*n3*n4*n5 doubles, one
+send and one receive per side on a periodic ring.
+
+This module is plumbing: it plans the slab (sizes, neighbours, the four halo regions), moves halos with
+torch.distributed point-to-point calls (NCCL on GPUs, gloo in the CPU tests) or, for one process holding several
+slabs, with device copies, and sequences C-ABI calls.  Every arithmetic step runs in libbsl6d.so:
+  * interior context: grid (L, n1..n5) on the interior view of the local array -- sweeps along dims 1-5, rotate, density;
+  * x1 context: grid (L + 2w, n1..n5) with bsl6d_set_boundary(0, open) -- the x1 sweep over interior + halos.
+The interior results are bit-identical to the same operation on the undivided grid (tests/test_gpu_slab.py).
+Measured on hardware: single GPU only (this environment has one GPU per run); the N > 1 path is covered by the
+world_size-2 gloo test of the exchange and by the single-GPU emulation with 2 and 4 slabs.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+import torch
+
+from . import api
+
+
+@dataclass(frozen=True)
+class SlabPlan:
+    """Host-side geometry of one rank's slab (no device state)."""
+    n_global: tuple
+    world: int
+    rank: int
+    q: int
+    L: int                 # interior planes of this rank
+    w: int                 # halo planes per side
+    plane: int             # doubles per x1 plane = n1*n2*n3*n4*n5
+    left: int              # ring neighbours
+    right: int
+
+    @property
+    def local_shape(self):
+        return (self.L + 2 * self.w,) + tuple(self.n_global[1:])
+
+    @property
+    def x1_offset(self) -> int:
+        """Global x1 index of the first interior plane."""
+        return self.rank * self.L
+
+    # plane ranges [lo, hi) inside the local array
+    @property
+    def interior(self):
+        return (self.w, self.w + self.L)
+
+    @property
+    def send_lo(self):      # my lowest interior planes -> the LEFT neighbour's upper halo
+        return (self.w, 2 * self.w)
+
+    @property
+    def send_hi(self):      # my highest interior planes -> the RIGHT neighbour's lower halo
+        return (self.L, self.L + self.w)
+
+    @property
+    def recv_lo(self):      # lower halo <- the LEFT neighbour's send_hi
+        return (0, self.w)
+
+    @property
+    def recv_hi(self):      # upper halo <- the RIGHT neighbour's send_lo
+        return (self.w + self.L, 2 * self.w + self.L)
+
+    @property
+    def halo_bytes_per_side(self) -> int:
+        return 8 * self.w * self.plane
+
+
+def plan_slab(n_global: Sequence[int], degree: int, world: int, rank: int, max_shift_cells: float) -> SlabPlan:
+    """Halo width: the stencil reaches q/2 nodes beyond the foot cell and the foot lies up to ceil(max|alpha|) cells
+    away (k = floor(alpha) in [-ceil, ceil-1]).  The halo must come from the direct neighbours: w <= L."""
+    n = tuple(int(v) for v in n_global)
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("bad world/rank")
+    if n[0] % world:
+        raise ValueError(f"n0 = {n[0]} is not divisible by {world} ranks (PAPER.md:148: points per dim a multiple of "
+                         f"the ranks per dim)")
+    q = int(degree) + 1
+    L = n[0] // world
+    w = q // 2 + int(math.ceil(abs(float(max_shift_cells))))
+    if w > L:
+        raise ValueError(f"halo width {w} exceeds the slab thickness {L}: use fewer ranks or a smaller time step")
+    plane = 1
+    for v in n[1:]:
+        plane *= v
+    return SlabPlan(n, world, rank, q, L, w, plane, (rank - 1) % world, (rank + 1) % world)
+
+
+def _planes(t: torch.Tensor, r):
+    return t[r[0]:r[1]]
+
+
+def exchange_local(plans: List[SlabPlan], locals_: List[torch.Tensor]) -> None:
+    """One process holds every slab of the ring (tests; single-GPU emulation): halo exchange by device copies,
+    one copy per halo (contiguous blocks)."""
+    R = len(plans)
+    for r in range(R):
+        p = plans[r]
+        _planes(locals_[r], p.recv_lo).copy_(_planes(locals_[p.left], plans[p.left].send_hi))
+        _planes(locals_[r], p.recv_hi).copy_(_planes(locals_[p.right], plans[p.right].send_lo))
+
+
+def exchange(plan: SlabPlan, f_local: torch.Tensor, group=None):
+    """Periodic-ring halo exchange with the two neighbours over torch.distributed (one send and one receive per side,
+    posted together).  Returns after the halos of f_local are filled."""
+    import torch.distributed as dist
+    if plan.world == 1:
+        _planes(f_local, plan.recv_lo).copy_(_planes(f_local, plan.send_hi))
+        _planes(f_local, plan.recv_hi).copy_(_planes(f_local, plan.send_lo))
+        return
+    ops = [
+        dist.P2POp(dist.isend, _planes(f_local, plan.send_hi), plan.right, group, tag=1),
+        dist.P2POp(dist.irecv, _planes(f_local, plan.recv_lo), plan.left, group, tag=1),
+        dist.P2POp(dist.isend, _planes(f_local, plan.send_lo), plan.left, group, tag=2),
+        dist.P2POp(dist.irecv, _planes(f_local, plan.recv_hi), plan.right, group, tag=2),
+    ]
+    # With two ranks both neighbours are the same peer.  Every rank posts the same order (hi out, lo in, lo out, hi in),
+    # so NCCL's in-order matching per peer pairs my first send with the peer's first receive (gloo matches by tag).
+    reqs = dist.batch_isend_irecv(ops)
+    for r in reqs:
+        r.wait()
+
+
+class Slab:
+    """One rank's slab: plan + the two library contexts (created on first use; needs a CUDA device)."""
+
+    def __init__(self, n_global, lo, dx, degree: int, world: int, rank: int, max_shift_cells: float):
+        self.plan = plan_slab(n_global, degree, world, rank, max_shift_cells)
+        self.lo, self.dx, self.degree = tuple(lo), tuple(dx), int(degree)
+        self._int: Optional[api.Context] = None
+        self._x1: Optional[api.Context] = None
+
+    # -- contexts ------------------------------------------------------------------------------------------
+    @property
+    def ctx_interior(self) -> api.Context:
+        if self._int is None:
+            p = self.plan
+            lo = (self.lo[0] + p.x1_offset * self.dx[0],) + self.lo[1:]
+            self._int = api.create((p.L,) + tuple(p.n_global[1:]), lo, self.dx, self.degree)
+        return self._int
+
+    @property
+    def ctx_x1(self) -> api.Context:
+        if self._x1 is None:
+            p = self.plan
+            lo = (self.lo[0] + (p.x1_offset - p.w) * self.dx[0],) + self.lo[1:]
+            self._x1 = api.create(p.local_shape, lo, self.dx, self.degree)
+            self._x1.set_boundary(0, True)
+        return self._x1
+
+    def destroy(self):
+        for c in (self._int, self._x1):
+            if c is not None:
+                c.destroy()
+        self._int = self._x1 = None
+
+    # -- storage -------------------------------------------------------------------------------------------
+    def alloc(self, device="cuda") -> torch.Tensor:
+        return torch.zeros(self.plan.local_shape, dtype=torch.float64, device=device)
+
+    def interior(self, f_local: torch.Tensor) -> torch.Tensor:
+        lo, hi = self.plan.interior
+        return f_local[lo:hi]
+
+    def scatter_from_global(self, f_global: torch.Tensor, f_local: torch.Tensor) -> torch.Tensor:
+        p = self.plan
+        self.interior(f_local).copy_(f_global[p.x1_offset:p.x1_offset + p.L])
+        return f_local
+
+    # -- operations (the halos of f_local must be current for advect_x1) ---------------------------------------
+    def advect_x1(self, f_local: torch.Tensor, dt: float, max_check: bool = True):
+        """x1 sweep over the whole local array, in place; interior results are exact, halo planes become stale."""
+        if max_check:
+            vmax = max(abs(self.lo[3]), abs(self.lo[3] + (self.plan.n_global[3] - 1) * self.dx[3]))
+            need = self.plan.q // 2 + int(math.ceil(vmax * abs(dt) / self.dx[0]))
+            if need > self.plan.w:
+                raise ValueError(f"displacement of {vmax * abs(dt) / self.dx[0]:.2f} cells needs {need} halo planes, "
+                                 f"the slab has {self.plan.w}")
+        self.ctx_x1.advect(f_local, f_local, 0, None, dt)
+
+    def advect(self, f_local: torch.Tensor, dim: int, shift_source, dt: float):
+        """Sweep along dim 1..5 on the interior, in place (E sources are over this rank's x points)."""
+        assert 1 <= dim <= 5
+        v = self.interior(f_local)
+        self.ctx_interior.advect(v, v, dim, shift_source, dt)
+
+    def rotate(self, f_local: torch.Tensor, B, dt: float):
+        v = self.interior(f_local)
+        self.ctx_interior.rotate(v, v, B, dt)
+
+    def density(self, f_local: torch.Tensor, rho: torch.Tensor):
+        return self.ctx_interior.density(self.interior(f_local), rho)
+
+    def strang_step(self, f_local: torch.Tensor, E, B, dt: float, exchange_fn):
+        """x1,x2,x3 (dt/2) -> v1,v2,v3 with E (dt) -> rotation -> x1,x2,x3 (dt/2); exchange_fn(f_local) refreshes the
+        halos (it is called before each of the two x1 sweeps).  E: three tensors over THIS rank's (L, n1, n2) x points."""
+        half = 0.5 * dt
+        v = self.interior(f_local)
+        ci = self.ctx_interior
+        exchange_fn(f_local)
+        self.advect_x1(f_local, half)
+        seq = [(1, None, 0, half / self.dx[1]), (2, None, 0, half / self.dx[2])]
+        if E is not None:
+            seq += [(3 + d, E[d], 0x7, dt / self.dx[3 + d]) for d in range(3) if E[d] is not None]
+        ci.advect_seq(v, v, seq)
+        if B is not None:
+            ci.rotate(v, v, B, dt)
+        exchange_fn(f_local)
+        self.advect_x1(f_local, half)
+        ci.advect_seq(v, v, [(1, None, 0, half / self.dx[1]), (2, None, 0, half / self.dx[2])])
