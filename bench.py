@@ -61,6 +61,9 @@ def parse_args():
     p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     p.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     p.add_argument("--no-fused", action="store_true", help="skip the fused-pass variant of the step")
+    p.add_argument("--sharded", action="store_true",
+                   help="instead of N replicas: ONE global grid cut into x1 slabs over the N ranks, with the ring halo "
+                        "exchange before every x1 sweep (strong scaling; DESIGN.md section 7)")
     p.add_argument("--paper-benchmark", action="store_true",
                    help="instead of the contract step: the paper's own section-5 benchmark (37^6, random per-point "
                         "shifts, odd widths 3/5/7/9, every direction) through bsl6d_advect_pointwise")
@@ -617,6 +620,66 @@ def run_ours(args, w, extra):
         G.dist.destroy_process_group()
 
 
+def run_sharded(args, w):
+    """One global grid, x1 slabs over the ranks (paper_2303_05994_b200/slab.py): a step is the Strang step of the
+    workload through Slab.strang_step -- halo exchange (NCCL point-to-point, or a device copy with one rank) before
+    each of the two x1 sweeps -- plus the density moment.  `value` counts the global grid's point updates."""
+    G = Gpu()
+    torch = G.torch
+    from paper_2303_05994_b200 import slab
+    K, W = args.steps, args.warmup
+    B, dt = (w.B, w.dt) if any(w.B) else (ROT_B, w.dt)
+    vmax = max(abs(w.lo[3]), abs(w.lo[3] + (w.n[3] - 1) * w.dx[3]))
+    s = slab.Slab(w.n, w.lo, w.dx, w.degree, G.world, G.rank, vmax * 0.5 * dt / w.dx[0])
+    p = s.plan
+    f = s.alloc(G.dev)
+    sub = replace(w, n=(p.L,) + tuple(w.n[1:]), lo=(w.lo[0] + p.x1_offset * w.dx[0],) + tuple(w.lo[1:]))
+    sub.fill(s.interior(f))                               # this rank's planes of the seeded global f (noise differs
+    #                                                       from the undivided recipe only in its linear index origin)
+    E = [torch.from_numpy(e[p.x1_offset:p.x1_offset + p.L].copy()).to(G.dev) for e in w.E()]
+    rho = torch.empty((p.L,) + tuple(w.n[1:3]), dtype=torch.float64, device=G.dev)
+    ex = lambda t: slab.exchange(p, t)
+
+    def one_step():
+        s.strang_step(f, E, B, dt, ex)
+        s.density(f, rho)
+
+    for _ in range(max(W, 0)):
+        one_step()
+    G.barrier()
+    l0 = s.ctx_interior.launch_count() + s.ctx_x1.launch_count()
+    clocks = ClockSampler(G.local)
+    clocks.start()
+    time.sleep(0.25)
+    G.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(G.stream)
+    for _ in range(K):
+        one_step()
+    e1.record(G.stream)
+    G.barrier()
+    clk = clocks.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), G.dev)
+    launches = s.ctx_interior.launch_count() + s.ctx_x1.launch_count() - l0
+    assert torch.isfinite(rho).all()
+    if G.rank == 0:
+        npts = w.npts
+        cfg = config_dict(w, G.world)
+        cfg["parallelism"] = (f"ONE global grid in x1 slabs over {G.world} rank(s): {p.L} planes + {p.w} halo planes per "
+                              f"side; ring halo exchange ({p.halo_bytes_per_side / 1e9:.2f} GB per side) before each x1 sweep")
+        line = {"metric": METRIC, "value": 12 * npts * K / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": G.world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clk, "gpu_launches": int(launches),
+                "halo_bytes_per_step_per_rank": 4 * p.halo_bytes_per_side, "fusion": "planner default",
+                "e2e": None, "roofline": None, "cpu_baseline": None,
+                "note": "sharded mode: the whole-job value of ONE grid; measured on hardware with one rank only in this "
+                        "environment"}
+        print(json.dumps(line), flush=True)
+    s.destroy()
+    if G.world > 1:
+        G.dist.destroy_process_group()
+
+
 def run_paper_benchmark(args):
     """one 1-D interpolation per direction on 37^6 points, random alpha/dx in [-1,1] per
     point, odd stencil widths.  Reports, per width and direction, the time and GB/s in the paper's convention
@@ -679,6 +742,9 @@ def main():
     w = wl.CONFIGS[args.workload or HEADLINE]
     if args.impl == "reference":
         run_reference(args, w)
+        return
+    if args.sharded:
+        run_sharded(args, w)
         return
     names = args.per_config if args.per_config is not None else ("C2,C3" if args.workload is None else "")
     extra = [wl.CONFIGS[n] for n in names.split(",") if n and n != w.name]

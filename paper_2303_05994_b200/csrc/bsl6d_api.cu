@@ -193,15 +193,17 @@ const void* generic_by_q(int q) {
 }
 const void* generic_fn(int q, int T) { return T == 64 ? generic_by_q<64>(q) : generic_by_q<32>(q); }
 
+constexpr int kGenericUnitSegments = 4;                      // threads per pencil in the unit-stride fallback
 template <int T>
 const void* generic_unit_by_q(int q) {
+    constexpr int S = kGenericUnitSegments;
     switch (q) {
-        case 2: return (const void*)bsl6d::sweep_generic_unit_kernel<2, T>;
-        case 4: return (const void*)bsl6d::sweep_generic_unit_kernel<4, T>;
-        case 6: return (const void*)bsl6d::sweep_generic_unit_kernel<6, T>;
-        case 8: return (const void*)bsl6d::sweep_generic_unit_kernel<8, T>;
-        case 10: return (const void*)bsl6d::sweep_generic_unit_kernel<10, T>;
-        case 12: return (const void*)bsl6d::sweep_generic_unit_kernel<12, T>;
+        case 2: return (const void*)bsl6d::sweep_generic_unit_kernel<2, T, S>;
+        case 4: return (const void*)bsl6d::sweep_generic_unit_kernel<4, T, S>;
+        case 6: return (const void*)bsl6d::sweep_generic_unit_kernel<6, T, S>;
+        case 8: return (const void*)bsl6d::sweep_generic_unit_kernel<8, T, S>;
+        case 10: return (const void*)bsl6d::sweep_generic_unit_kernel<10, T, S>;
+        case 12: return (const void*)bsl6d::sweep_generic_unit_kernel<12, T, S>;
         default: return nullptr;
     }
 }
@@ -223,7 +225,9 @@ int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     int T = 64;
     if (per_thread * T > cap) T = 32;
     if (per_thread * T > cap) return BSL6D_EUNSUPPORTED;
-    k = KernelChoice{nullptr, T, per_thread * T, 2, T};
+    // gen_T = pencils per block; the unit-stride fallback runs kGenericUnitSegments threads per pencil
+    const bool unit = inner == 1 && !periodic;
+    k = KernelChoice{nullptr, unit ? T * kGenericUnitSegments : T, per_thread * T, 2, T};
     return BSL6D_OK;
 }
 
@@ -364,7 +368,7 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
         int per = is_periodic(c, dim) ? 1 : 0;
         void* gargs[] = {(void*)&a, (void*)&per};                  // the unit-stride kernel takes only `a`
         grid = (unsigned)((inner * outer + (size_t)kc.gen_T - 1) / (size_t)kc.gen_T);
-        e = cudaLaunchKernel(gfn, dim3(grid), dim3(kc.gen_T), gargs, kc.smem, stream);
+        e = cudaLaunchKernel(gfn, dim3(grid), dim3(kc.threads), gargs, kc.smem, stream);
         if (e != cudaSuccess) return cuda_fail(c, e);
     } else {
         rc = allow_smem(c, (const void*)kc.fn, kc.smem);
@@ -513,27 +517,42 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
         rc = choose_kernel(c, sw[i].dim, kc);
         if (rc) return rc;
     }
-    // Fewest passes over the chain (dynamic programme from the back): a group of 3 (a,b,a), 2 (a,b) or 1 sweeps.
-    // pick[i] > 0: a two-dim tile pass over that many sweeps (or a single sweep); pick[i] < 0: a whole-v-block pass
-    // over -pick[i] sweeps.  Ties go to the later candidate: v-block pass > triple > pair > single.
-    std::vector<int> best(ns + 1, 0), pick(ns + 1, 1);
+    // Cheapest plan over the chain (dynamic programme from the back).  Costs are in units of ONE single sweep of the
+    // same grid (a 16 B/point pass at HBM speed) and come from the per-pass timings of DESIGN.md section 10
+    // (C2: q = 8, C5: q = 10, in-step medians); they only have to rank the alternatives:
+    //   single sweep                      1
+    //   persistent tile pass, n sweeps    0.45 + (0.035 q + 0.07) n      (+0.3 when an extent exceeds 32: two buffers)
+    //   v-block pass, n sweeps            0.90 + (0.020 q + 0.03) n      (+1 per v3 sweep: distributed shared memory)
+    //   round-1 tile kernels              pair 0.7 + 0.10 q,  a-b-a triple 0.7 + 0.13 q
+    // Fusion mode 2 ("wherever a kernel exists") counts passes instead: every pass costs 1, ties go to the larger group.
+    // pick[i] > 0: a round-1 tile pass over that many sweeps (or a single sweep); pick[i] >= 100: a persistent tile pass
+    // over pick[i]-100 sweeps; pick[i] < 0: a v-block pass over -pick[i] sweeps.
+    const double q = (double)c->q;
+    const bool by_count = c->fuse_all != 0;
+    const double eps = 1e-9;
+    std::vector<double> best(ns + 1, 0.0);
+    std::vector<int> pick(ns + 1, 1);
     std::vector<Pass> cand2(ns), cand3(ns), candv(ns), candp(ns);
-    std::vector<int> plen(ns, 0);
+    auto better = [&](double total, double cur) { return total < cur - eps || (by_count && total < cur + eps); };
     for (int i = ns - 1; i >= 0; --i) {
-        best[i] = 1 + best[i + 1];
+        best[i] = 1.0 + best[i + 1];
         pick[i] = 1;
         if (c->fusion && c->use_fused && i + 1 < ns && try_fuse(c, sw, i, 2, cand2[i])) {
-            if (1 + best[i + 2] < best[i]) { best[i] = 1 + best[i + 2]; pick[i] = 2; }
+            const double total = (by_count ? 1.0 : 0.7 + 0.10 * q) + best[i + 2];
+            if (total < best[i] - eps) { best[i] = total; pick[i] = 2; }
         }
         if (c->fusion && c->use_fused && i + 2 < ns && try_fuse(c, sw, i, 3, cand3[i])) {
-            if (1 + best[i + 3] < best[i]) { best[i] = 1 + best[i + 3]; pick[i] = 3; }
+            const double total = (by_count ? 1.0 : 0.7 + 0.13 * q) + best[i + 3];
+            if (total < best[i] - eps) { best[i] = total; pick[i] = 3; }
         }
         if (c->fusion && c->use_ptile) {
-            // persistent tile passes: ties with the round-1 kernels go to these, longer chains win
             for (int len = 2; len <= bsl6d::kMaxPSweeps && i + len <= ns; ++len) {
                 Pass p;
                 if (!try_ptile(c, sw, i, len, p)) break;      // a third dim (or the unit-stride dim) ends the chain
-                if (1 + best[i + len] <= best[i]) { best[i] = 1 + best[i + len]; pick[i] = 100 + len; candp[i] = p; }
+                const bool big = p.pc.na > 32 || p.pc.nb > 32;
+                const double cost = by_count ? 1.0 : 0.45 + (0.035 * q + 0.07) * len + (big ? 0.3 : 0.0);
+                const double total = cost + best[i + len];
+                if (better(total, best[i])) { best[i] = total; pick[i] = 100 + len; candp[i] = p; }
             }
         }
         if (c->fusion && c->use_vblock) {
@@ -541,13 +560,15 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
             while (i + run < ns && sw[i + run].dim >= 3 && (c->fuse_all || sw[i + run].dim != 5) &&
                    run < bsl6d::kMaxVSweeps)
                 ++run;
-            for (int len = c->vblock_min; len <= run; ++len) {
+            int n_v3 = 0;
+            for (int len = 1; len <= run; ++len) {
+                n_v3 += sw[i + len - 1].dim == 5 ? 1 : 0;
+                if (len < c->vblock_min) continue;
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
-                // Measured: for three or more sweeps the v-block kernel (two CTAs per SM, swizzled
-                // tile) is at least as fast as the persistent tile pass, for a pair the persistent pass wins.
-                const int total = 1 + best[i + len];
-                if (total < best[i] || (total == best[i] && len >= 3)) { best[i] = total; pick[i] = -len; candv[i] = p; }
+                const double cost = by_count ? 1.0 : 0.90 + (0.020 * q + 0.03) * len + 1.0 * n_v3;
+                const double total = cost + best[i + len];
+                if (better(total, best[i])) { best[i] = total; pick[i] = -len; candv[i] = p; }
             }
         }
     }

@@ -340,42 +340,49 @@ __global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int
     }
 }
 
-// The same for the unit-stride dim (inner == 1; always a v dim => zero extension): a block owns T consecutive
+// The same for the unit-stride dim (inner == 1; always a v dim => zero extension): a block owns PB consecutive
 // pencils = one contiguous chunk, moved coalesced through two shared-memory tiles (input rows, output rows) with an
-// odd row pitch, so that "lane = pencil" accesses are conflict-free.
-template <int Q, int T>
-__global__ void __launch_bounds__(T) sweep_generic_unit_kernel(const SweepArgs a) {
-    extern __shared__ double tile[];                       // 2 * T * LD
+// odd row pitch, so that "lane = pencil" accesses are conflict-free.  A pencil is cut into S segments of
+// ceil(n/S) outputs, one thread each (the lanes of a warp share the segment), which gives a block S times the warps
+// for the same tile (with one thread per pencil the kernel ran 10 warps per SM: 3.4 TB/s at 36^6).
+template <int Q, int PB, int S>
+__global__ void __launch_bounds__(PB * S) sweep_generic_unit_kernel(const SweepArgs a) {
+    extern __shared__ double tile[];                       // 2 * PB * LD
+    constexpr int T = PB * S;
     const int n = (int)a.n;
     const int LD = n | 1;
     double* tin = tile;
-    double* tout = tile + (size_t)T * LD;
-    const size_t p0 = (size_t)blockIdx.x * T;
-    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)T ? ((size_t)a.outer - p0) : (size_t)T);
+    double* tout = tile + (size_t)PB * LD;
+    const size_t p0 = (size_t)blockIdx.x * PB;
+    const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)PB ? ((size_t)a.outer - p0) : (size_t)PB);
     const uint32_t nelem = np * (uint32_t)n;
     const double* pin = a.in + p0 * n;
     double* pout = a.out + p0 * n;
     for (uint32_t e = threadIdx.x; e < nelem; e += T) tin[(e / n) * LD + (e % n)] = __ldcs(pin + e);
     __syncthreads();
-    if (threadIdx.x < np) {
+    const uint32_t pl = threadIdx.x % PB;
+    const int seg = (int)(threadIdx.x / PB);
+    if (pl < np) {
         long long k;
         double theta;
-        split_shift(__ldg(a.src + src_offset(a.terms, (uint32_t)(p0 + threadIdx.x), 0u)), a.scale, k, theta);
+        split_shift(__ldg(a.src + src_offset(a.terms, (uint32_t)(p0 + pl), 0u)), a.scale, k, theta);
         double w[Q];
         lagrange_weights<Q>(theta, w);
+        const int R = (n + S - 1) / S;
+        const int j0 = seg * R, j1 = (j0 + R < n) ? j0 + R : n;
         const long long lim = 2LL * n + 32;
         long long kk = k + (long long)(1 - Q / 2);
         kk = kk < -lim ? -lim : (kk > lim ? lim : kk);
-        int row = (int)kk;
-        const double* rin = tin + threadIdx.x * LD;
-        double* rout = tout + threadIdx.x * LD;
+        int row = (int)kk + j0;                            // first stencil node of output j0
+        const double* rin = tin + pl * LD;
+        double* rout = tout + pl * LD;
         double win[Q];
 #pragma unroll
         for (int m = 0; m < Q - 1; ++m) {
             win[m + 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
             ++row;
         }
-        for (int j = 0; j < n; ++j) {
+        for (int j = j0; j < j1; ++j) {
 #pragma unroll
             for (int m = 0; m < Q - 1; ++m) win[m] = win[m + 1];
             win[Q - 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
