@@ -494,9 +494,9 @@ bool try_vblock(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p
     if (cnt < 2 || cnt > bsl6d::kMaxVSweeps) return false;
     for (int k = 0; k < cnt; ++k) {
         if (sw[i + k].dim < 3) return false;
-        // Policy from measurement: a v3 sweep inside the pass crosses the cluster through
-        // distributed shared memory (~16 B/clk per SM at best, ~3 clk per scattered 8-byte request) and costs more
-        // than the v3 sweep as a pass of its own; only fusion mode 2 takes it.
+        // Policy from measurement: a v3 sweep inside the pass needs the block in the other cut
+        // (re-tiled through L2: store, cluster barrier, reload -- or, slower still, read through distributed shared
+        // memory) and costs more than the v3 sweep as a pass of its own; only fusion mode 2 takes it.
         if (sw[i + k].dim == 5 && !c->fuse_all) return false;
     }
     const int32_t* n = c->g.n;
@@ -522,7 +522,8 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
     // (C2: q = 8, C5: q = 10, in-step medians); they only have to rank the alternatives:
     //   single sweep                      1
     //   persistent tile pass, n sweeps    0.45 + (0.035 q + 0.07) n      (+0.3 when an extent exceeds 32: two buffers)
-    //   v-block pass, n sweeps            0.90 + (0.020 q + 0.03) n      (+1 per v3 sweep: distributed shared memory)
+    //   v-block pass, n sweeps            0.90 + (0.020 q + 0.03) n      (+1.3 per switch between v1/v2 sweeps and v3
+    //                                                                      sweeps: the block is re-tiled through L2)
     //   round-1 tile kernels              pair 0.7 + 0.10 q,  a-b-a triple 0.7 + 0.13 q
     // Fusion mode 2 ("wherever a kernel exists") counts passes instead: every pass costs 1, ties go to the larger group.
     // pick[i] > 0: a round-1 tile pass over that many sweeps (or a single sweep); pick[i] >= 100: a persistent tile pass
@@ -560,13 +561,13 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
             while (i + run < ns && sw[i + run].dim >= 3 && (c->fuse_all || sw[i + run].dim != 5) &&
                    run < bsl6d::kMaxVSweeps)
                 ++run;
-            int n_v3 = 0;
+            int switches = 0;
             for (int len = 1; len <= run; ++len) {
-                n_v3 += sw[i + len - 1].dim == 5 ? 1 : 0;
+                if (len > 1 && (sw[i + len - 1].dim == 5) != (sw[i + len - 2].dim == 5)) ++switches;
                 if (len < c->vblock_min) continue;
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
-                const double cost = by_count ? 1.0 : 0.90 + (0.020 * q + 0.03) * len + 1.0 * n_v3;
+                const double cost = by_count ? 1.0 : 0.90 + (0.020 * q + 0.03) * len + 1.3 * switches;
                 const double total = cost + best[i + len];
                 if (better(total, best[i])) { best[i] = total; pick[i] = -len; candv[i] = p; }
             }

@@ -44,10 +44,27 @@ bool make_map(CUtensorMap* m, const double* f, uint32_t nx, int nv, int cw) {
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+#ifndef BSL6D_TUNE_V3PATH
+#define BSL6D_TUNE_V3PATH kV3ViaL2
+#endif
+
 template <int NV, int Q, int CL, int MINB>
 VBlockChoice choice() {
     using G = VBlockGeom<NV, CL>;
-    return VBlockChoice{(const void*)vblock_kernel<NV, Q, CL, MINB>, G::T, G::kSmemBytes, CL, G::CW};
+    return VBlockChoice{(const void*)vblock_kernel<NV, Q, CL, MINB, BSL6D_TUNE_V3PATH>, G::T, G::kSmemBytes, CL, G::CW};
+}
+
+// The other cut of the same block: box = [1][nv/cl j1-planes][nv][16 doubles], 128-byte half rows, 128B swizzle.
+bool make_map_b(CUtensorMap* m, const double* f, uint32_t nx, int nv, int cl) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)nv, (cuuint64_t)nv, (cuuint64_t)nv, (cuuint64_t)nx};
+    const cuuint64_t strides[3] = {(cuuint64_t)nv * 8, (cuuint64_t)nv * nv * 8, (cuuint64_t)nv * nv * nv * 8};
+    const cuuint32_t box[4] = {16u, (cuuint32_t)nv, (cuuint32_t)(nv / cl), 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(f), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 #ifndef BSL6D_TUNE_VCL
@@ -82,9 +99,15 @@ bool vblock_lookup(int nv1, int nv2, int nv3, int q, VBlockChoice& out) {
 
 cudaError_t vblock_launch(const VBlockChoice& vc, const double* f_in, double* f_out, uint32_t nx, int nv,
                           const VBlockArgs& args, cudaStream_t stream) {
-    CUtensorMap tin, tout;
+    CUtensorMap tin, tout, tinb, toutb;
     if (!make_map(&tin, f_in, nx, nv, vc.cw) || !make_map(&tout, f_out, nx, nv, vc.cw)) return cudaErrorInvalidValue;
-    void* kargs[] = {(void*)&tin, (void*)&tout, (void*)&args};
+    if (vc.cl > 1 && nv >= 16) {
+        if (!make_map_b(&tinb, f_in, nx, nv, vc.cl) || !make_map_b(&toutb, f_out, nx, nv, vc.cl)) return cudaErrorInvalidValue;
+    } else {
+        tinb = tin;                                        // unused by a single-CTA block
+        toutb = tout;
+    }
+    void* kargs[] = {(void*)&tin, (void*)&tout, (void*)&tinb, (void*)&toutb, (void*)&args};
     return cudaLaunchKernel(vc.fn, dim3(nx * (unsigned)vc.cl), dim3((unsigned)vc.threads), kargs, vc.smem, stream);
 }
 

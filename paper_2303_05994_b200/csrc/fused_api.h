@@ -26,7 +26,7 @@ bool fused_lookup_q10(int na, int nb, bool pa, bool pb, int pattern, FusedChoice
 namespace bsl6d {
 struct VBlockArgs;
 struct VBlockChoice {
-    const void* fn;        // __global__ void (*)(CUtensorMap, CUtensorMap, VBlockArgs)
+    const void* fn;        // __global__ void (*)(CUtensorMap in, out, in (other cut), out (other cut), VBlockArgs)
     int threads;
     size_t smem;
     int cl;                // CTAs per cluster = CTAs per v-block

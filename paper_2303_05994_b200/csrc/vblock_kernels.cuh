@@ -9,9 +9,11 @@
 //
 //   v1 / v2 sweeps  thread owns the pencil (j2,c) / (j1,c): whole pencil -> registers in shifted order ->
 //                   Q-term FMA chains -> back into the tile.  Entirely CTA-local.
-//   v3 sweeps       the pencil crosses the cluster.  Thread owns row pieces (j1,j2, this CTA's CW outputs); the
+//   v3 sweeps       the pencil crosses the cluster.  Default: the block is RE-TILED THROUGH L2 into the other cut
+//                   (each CTA: a quarter of the j1-planes, all of v3) by TMA stores / cluster barrier / TMA loads, the
+//                   sweep runs locally, and the block is re-tiled back.  Alternative (V3PATH = kV3ViaDsmem): the
 //                   CW+Q-1 inputs are read through distributed shared memory (mapa + ld.shared::cluster) from
-//                   whichever CTA owns the column; cluster barriers separate "everyone has read" from "write".
+//                   whichever CTA owns the column.  Both are measured slower than a v3 pass of its own (section 10).
 //
 // The tile rows are CW*8 = 64 or 128 bytes, written by the TMA with the matching 64B / 128B swizzle (16-byte chunk
 // index XOR row bits), which is what makes the v3 sweeps (lanes along rows) and the v1/v2 sweeps (lanes along c)
@@ -134,34 +136,100 @@ struct VBlockGeom {
     static_assert(PLANE % 1024 == 0 || (RB == 64 && PLANE % 512 == 0), "j1 planes must not disturb the swizzle bits");
 };
 
-template <int NV, int Q, int CL, int MINB>
+// How a v3 sweep is served when the v-block is cut along v3 over CL > 1 CTAs:
+//   kV3ViaL2   (default) RE-TILE THROUGH L2.  The cluster stores its four [j1][j2][c] tiles (TMA store to f_out, which
+//              lands in the 126 MB L2), synchronises, and every CTA loads the block again in the OTHER cut --
+//              [its NV/CL j1-planes][j2][all of v3], two TMA boxes of 128-byte half rows with the 128B swizzle -- runs the
+//              v3 sweep entirely locally (thread owns a row), stores, synchronises, and loads its [j1][j2][c] tile
+//              back.  Two extra round trips through L2 per v3 sweep (32 B/point of L2 traffic, none to HBM: the lines
+//              are still dirty in L2 and are overwritten there), all by bulk tensor copies.
+//   kV3ViaDsmem          the pencil's CW+Q-1 inputs are read from whichever CTA owns them through distributed shared
+//              memory (mapa + ld.shared::cluster) between cluster barriers.  Measured ~3 clk per scattered 8-byte
+//              request on B200: ~9 ms per v3 sweep at C2.  Kept for comparison.
+enum V3Path { kV3ViaL2 = 0, kV3ViaDsmem = 1 };
+
+template <int NV, int Q, int CL, int MINB, int V3PATH>
 __global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__((VBlockGeom<NV, CL>::T), MINB)
     vblock_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out,
+                  const __grid_constant__ CUtensorMap tm_inB, const __grid_constant__ CUtensorMap tm_outB,
                   const __grid_constant__ VBlockArgs a) {
     using G = VBlockGeom<NV, CL>;
     constexpr int CW = G::CW, RB = G::RB, PLANE = G::PLANE, T = G::T;
     constexpr uint32_t SWZ = G::SWZ;
+    constexpr bool RETILE = CL > 1 && V3PATH == kV3ViaL2;
+    // the other cut (RETILE only): BJ1 = NV/CL j1-planes x NV rows of NV doubles, as NV/16 boxes of 128-byte half rows
+    constexpr int BJ1 = NV / CL, BROWS = BJ1 * NV, BHALVES = (NV * 8) / 128, BBOX = BROWS * 128;
+    static_assert(!RETILE || (NV * 8) % 128 == 0, "re-tiling wants rows of whole 128-byte halves");
+    static_assert(!RETILE || BHALVES * BBOX == G::TILE, "both cuts fill the same buffer");
     extern __shared__ unsigned char vb_smem_raw[];
     __shared__ __align__(8) unsigned long long vb_mbar;
     const uint32_t tile = (vb::smem_u32(vb_smem_raw) + 1023u) & ~1023u;
     const uint32_t bar = vb::smem_u32(&vb_mbar);
     const uint32_t rank = CL > 1 ? (blockIdx.x % CL) : 0u;
     const uint32_t x = blockIdx.x / CL;
-    const int c_lo = (int)rank * CW;                       // first v3 index of this CTA
+    const int c_lo = (int)rank * CW;                       // first v3 index of this CTA (cut A)
 
     if (threadIdx.x == 0) {
         vb::mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        vb::mbar_expect_tx(bar, (uint32_t)G::TILE);
-        vb::tma_load_4d(tile, &tm_in, bar, c_lo, 0, 0, (int)x);
-    }
-    vb::mbar_wait(bar, 0);
+
+    uint32_t phase = 0;                                    // parity of the next TMA-load completion
+    bool stored = false;                                   // has the block been written to f_out yet?
+    int cut = -1;                                          // what the buffer holds: -1 nothing, 0 cut A, 1 cut B
+    auto load_cut = [&](int want) {
+        if (threadIdx.x == 0) {
+            vb::mbar_expect_tx(bar, (uint32_t)G::TILE);
+            if (want == 0) {
+                vb::tma_load_4d(tile, stored ? &tm_out : &tm_in, bar, c_lo, 0, 0, (int)x);
+            } else {
+#pragma unroll
+                for (int h = 0; h < BHALVES; ++h)
+                    vb::tma_load_4d(tile + h * BBOX, stored ? &tm_outB : &tm_inB, bar, 16 * h, 0, (int)rank * BJ1, (int)x);
+            }
+        }
+        vb::mbar_wait(bar, phase);
+        phase ^= 1u;
+        cut = want;
+    };
+    auto store_cut = [&](bool complete) {
+        // generic-proxy writes -> visible to the async proxy, then bulk store(s) of the buffer to f_out
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            if (cut == 0) {
+                vb::tma_store_4d(&tm_out, tile, c_lo, 0, 0, (int)x);
+            } else {
+#pragma unroll
+                for (int h = 0; h < BHALVES; ++h) vb::tma_store_4d(&tm_outB, tile + h * BBOX, 16 * h, 0, (int)rank * BJ1, (int)x);
+            }
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            if (complete) {
+                asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");     // the WRITES are done, not just the reads
+                asm volatile("fence.proxy.async;" ::: "memory");
+                __threadfence();
+            } else {
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            }
+        }
+        stored = true;
+    };
+    // switch the buffer to the cut the next sweep needs (RETILE): store, let the whole cluster finish storing, reload
+    auto want_cut = [&](int want) {
+        if (cut == want) return;
+        if (cut >= 0) {
+            store_cut(true);
+            cooperative_groups::this_cluster().sync();     // (also a CTA barrier: thread 0's store is complete for all)
+            asm volatile("fence.proxy.async;" ::: "memory");
+        }
+        load_cut(want);
+    };
 
     for (uint32_t s = 0; s < a.nsweeps; ++s) {
         const VSweep& sw = a.sw[s];
+        if (RETILE) want_cut(sw.dim == 5 ? 1 : 0);
+        else if (cut < 0) load_cut(0);
         if (sw.dim == 3) {
             // ---- along v1: pencil (j2, c), element j1 at  p_off + j1*PLANE  (swizzle term does not depend on j1)
             for (int p = threadIdx.x; p < NV * CW; p += T) {
@@ -195,8 +263,27 @@ __global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__((VBlockGeom<NV, CL>
                     vb::sts_f64(base + o + (c8 ^ (((o >> 7) & SWZ) << 4)), res[j]);
                 }
             }
+        } else if (RETILE) {
+            // ---- along v3, cut B: thread owns the whole row (j1 = rank*BJ1 + p/NV, j2 = p%NV); column col lives in half
+            // col/16 at  row*128 + ((col%16)*8 ^ (row&7)<<4)
+            for (int p = threadIdx.x; p < BROWS; p += T) {
+                const uint32_t rbase = tile + (uint32_t)p * 128u;
+                const uint32_t sx = ((uint32_t)p & 7u) << 4;
+                const uint32_t grow = (rank * BJ1 + (uint32_t)p / NV) * NV + (uint32_t)p % NV;      // j1*NV + j2
+                const double sval = __ldg(sw.src + src_offset(sw.terms, x * (NV * NV) + grow, 0u));
+                double res[NV];
+                vb::window_sweep<NV, NV, Q>(sval, sw.scale, 0,
+                                            [&](int col) {
+                                                const uint32_t h = (uint32_t)col >> 4, cl = (uint32_t)col & 15u;
+                                                return vb::lds_f64(rbase + h * BBOX + ((cl * 8) ^ sx));
+                                            },
+                                            res);
+#pragma unroll
+                for (int j = 0; j < NV; ++j)
+                    vb::sts_f64(rbase + (uint32_t)(j >> 4) * BBOX + (((uint32_t)(j & 15) * 8) ^ sx), res[j]);
+            }
         } else {
-            // ---- along v3: row piece (j1, j2) x this CTA's CW outputs; inputs from any CTA of the cluster
+            // ---- along v3, cut A: row piece (j1, j2) x this CTA's CW outputs; inputs from any CTA of the cluster
             // Hazard: a neighbour reads my boundary columns of row p while I want to overwrite row p.  Rows are
             // handled in RP rounds (round r = rows r*T .. r*T+T-1 in EVERY CTA of the cluster, each thread one row
             // piece); within a round everyone reads, the cluster synchronises, everyone writes.  Later rounds touch
@@ -230,15 +317,8 @@ __global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__((VBlockGeom<NV, CL>
         }
         __syncthreads();
     }
-
-    // generic-proxy writes -> visible to the async proxy, then one bulk store of the tile
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        vb::tma_store_4d(&tm_out, tile, c_lo, 0, 0, (int)x);
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-    }
+    if (cut < 0) load_cut(0);                              // an empty chain is a copy
+    store_cut(false);
 }
 
 }  // namespace bsl6d
