@@ -201,3 +201,36 @@ def test_oblique_B_rotation_matches_oracle(B, dt):
         ctx.rotate(inplace, inplace, B, dt)
     assert torch.equal(fused, plain) and torch.equal(inplace, plain)
     assert rel_err(fused, oracle.rotate(ogrid(w), w.degree, f, B, dt)) <= TOL
+
+
+def test_strang_step_is_capturable_in_a_cuda_graph():
+    """Every entry point only enqueues work on the caller's stream (no allocation, no synchronisation in steady state),
+    so a launch-bound loop of small steps can be captured once and replayed as a CUDA graph (C1 is 2 MiB: L2-resident,
+    launch-latency-bound).  Replays must reproduce eager execution bit for bit -- persistent TMA-fed passes included."""
+    _need_gpu()
+    w = wl.C2.reduced((8, 8, 8, 16, 16, 16))
+    f0 = w.make_f("cuda")
+    Ed = [torch.from_numpy(e).cuda() for e in w.E()]
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        eager = f0.clone()
+        tmp = torch.empty_like(eager)
+        for _ in range(4):
+            ctx.strang_step(eager, tmp, Ed, w.B if any(w.B) else (0.0, 0.0, 1.0), w.dt)
+        g_f = f0.clone()
+        g_tmp = torch.empty_like(g_f)
+        B = w.B if any(w.B) else (0.0, 0.0, 1.0)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):                           # warm-up on the capture stream (first-use attributes)
+            ctx.strang_step(g_f, g_tmp, Ed, B, w.dt, stream=side)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g_f.copy_(f0)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            ctx.strang_step(g_f, g_tmp, Ed, B, w.dt, stream=torch.cuda.current_stream())
+        g_f.copy_(f0)
+        for _ in range(4):
+            graph.replay()
+        torch.cuda.synchronize()
+    assert torch.equal(g_f, eager)
