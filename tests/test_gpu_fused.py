@@ -234,3 +234,47 @@ def test_strang_step_is_capturable_in_a_cuda_graph():
             graph.replay()
         torch.cuda.synchronize()
     assert torch.equal(g_f, eager)
+
+
+@pytest.mark.parametrize("n,degree,seed", [((8, 8, 8, 8, 8, 8), 7, 1), ((4, 16, 16, 16, 16, 16), 5, 2),
+                                            ((2, 2, 32, 32, 32, 32), 9, 3), ((3, 32, 32, 32, 32, 8), 7, 4)])
+def test_random_chains_every_planner_mode_equals_single_sweeps(n, degree, seed):
+    """Random chains of sweeps (any order of dims, repeats, sources over random subsets of the other dims, displacements
+    of up to ~2.5 cells): whatever grouping the planner picks in modes 1-4 -- persistent tile passes with chains like
+    b,a,b,a, v-block passes with re-tiling, round-1 pairs and triples -- the result equals the sweeps launched one by
+    one, bit for bit, in place and out of place; and the first chain also agrees with the oracle."""
+    _need_gpu()
+    rng = np.random.default_rng(seed)
+    w = wl.replace(wl.C5.reduced(n), degree=degree)
+    f = w.make_f("cpu").numpy()
+    fd = torch.from_numpy(f).cuda()
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for trial in range(6):
+            ns = int(rng.integers(2, 11))
+            chain_host = []
+            dims = rng.integers(0, 6, size=ns) if trial % 2 else rng.choice([3, 4, 5, 3, 4, 2], size=ns)
+            for d in dims:
+                others = [k for k in range(6) if k != d]
+                mask = 0
+                for k in rng.choice(others, size=int(rng.integers(0, 3)), replace=False):
+                    mask |= 1 << int(k)
+                shape = [w.n[k] for k in range(6) if mask >> k & 1]
+                src = 2.5 * (2.0 * rng.random(shape if shape else (1,)) - 1.0)
+                chain_host.append((int(d), src, mask, 1.0))
+            chain = [(d, torch.from_numpy(np.ascontiguousarray(s)).cuda(), m, sc) for d, s, m, sc in chain_host]
+            ctx.set_fusion(0)
+            single = ctx.advect_seq(fd, torch.empty_like(fd), chain)
+            for mode in (1, 2, 3, 4):
+                ctx.set_fusion(mode)
+                npass = ctx.seq_passes(chain)
+                assert 1 <= npass <= ns
+                out = ctx.advect_seq(fd, torch.empty_like(fd), chain)
+                assert torch.equal(out, single), (trial, mode, [c[0] for c in chain_host])
+                inp = fd.clone()
+                ctx.advect_seq(inp, inp, chain)
+                assert torch.equal(inp, single), (trial, mode, "in place")
+            if trial == 0:
+                ref = f
+                for d, s, m, sc in chain_host:
+                    ref = oracle.sweep(ref, d, np.ascontiguousarray(s), m, sc, w.degree + 1)
+                assert rel_err(single, ref) <= TOL
