@@ -195,24 +195,39 @@ __global__ void __launch_bounds__((PTileGeom<NA, NB>::THREADS), 1)
         const uint32_t ch = t % a.nchunks, om = t / a.nchunks;
         const uint32_t m = om % a.mid, o = om / a.mid;
         const uint32_t i0 = ch * C;
+
+        // The shift source of a pencil is a (small, cached) global load at the head of every sweep: a dependent
+        // latency of several hundred cycles per sweep with only four warps per scheduler to cover it.  The value for
+        // the thread's first pencil of sweep s+1 is therefore fetched while sweep s runs (and the one for sweep 0
+        // while the tile is still in flight).
+        auto shift_source = [&](uint32_t s, int p) -> double {
+            const PSweep& sw = a.sw[s];
+            if (!sw.along_b) {
+                // pencil (i_b, c) along a: a-view of the array has outer index o, inner index (m*NB + i_b)*inner_b + i
+                const uint32_t ib = (uint32_t)p / C, c = (uint32_t)p % C;
+                return __ldg(sw.src + src_offset(sw.terms, o, (m * NB + ib) * a.inner_b + i0 + c));
+            }
+            // pencil (i_a, c) along b: b-view has outer index (o*NA + i_a)*mid + m, inner index i
+            const uint32_t ia = (uint32_t)p / C, c = (uint32_t)p % C;
+            return __ldg(sw.src + src_offset(sw.terms, (o * NA + ia) * a.mid + m, i0 + c));
+        };
+        double sval_next = 0.0;
+        if (a.nsweeps > 0 && gt < (a.sw[0].along_b ? NA * C : NB * C)) sval_next = shift_source(0, gt);
         pt::mbar_wait(full0 + 8 * (2 * b + (use & 1)), (use >> 1) & 1);
 
         for (uint32_t s = 0; s < a.nsweeps; ++s) {
             const PSweep& sw = a.sw[s];
+            const double sval_first = sval_next;
+            if (s + 1 < a.nsweeps && gt < (a.sw[s + 1].along_b ? NA * C : NB * C)) sval_next = shift_source(s + 1, gt);
             if (!sw.along_b) {
-                // pencil (i_b, c) along a: a-view of the array has outer index o, inner index (m*NB + i_b)*inner_b + i
                 for (int p = gt; p < NB * C; p += GT) {
-                    const uint32_t ib = (uint32_t)p / C, c = (uint32_t)p % C;
-                    const uint32_t inner_idx = (m * NB + ib) * a.inner_b + i0 + c;
-                    const double sval = __ldg(sw.src + src_offset(sw.terms, o, inner_idx));
+                    const double sval = p == gt ? sval_first : shift_source(s, p);
                     pt::pencil_in_place<NA, Q, PA, (uint32_t)PLANE>(buf + (uint32_t)p * 8u, sval, sw.scale);
                 }
             } else {
-                // pencil (i_a, c) along b: b-view has outer index (o*NA + i_a)*mid + m, inner index i
                 for (int p = gt; p < NA * C; p += GT) {
                     const uint32_t ia = (uint32_t)p / C, c = (uint32_t)p % C;
-                    const uint32_t outer_idx = (o * NA + ia) * a.mid + m;
-                    const double sval = __ldg(sw.src + src_offset(sw.terms, outer_idx, i0 + c));
+                    const double sval = p == gt ? sval_first : shift_source(s, p);
                     pt::pencil_in_place<NB, Q, PB, (uint32_t)ROW>(buf + ia * (uint32_t)PLANE + c * 8u, sval, sw.scale);
                 }
             }
