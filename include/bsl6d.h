@@ -157,8 +157,9 @@ BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* 
  * PAPER.md:84).  alpha_cells is a DEVICE array with the shape and layout of f: "the most general way to define the
  * interpolation shift is as a function of the full phase space" -- this is the kernel of the paper's
  * own section-5 benchmark (random alpha/dx in [-1,1], widths 3/5/7/9, 37^6 points).  A sweep moves
- * 24 B/point.  q in {3,5,7,9}; extents of `dim` in {8,16,32,37} (else BSL6D_EUNSUPPORTED).  f_in == f_out is legal;
- * alpha_cells must not overlap f_out. */
+ * 24 B/point.  q odd, 1..11 (else BSL6D_EUNSUPPORTED); any extent: kernels compiled per extent for q in {3,5,7,9} and
+ * extents {8,16,32,37,48,64}, run-time-extent kernels otherwise (unit-stride dim: extent <= ~400, else
+ * BSL6D_EUNSUPPORTED).  f_in == f_out is legal; alpha_cells must not overlap f_out. */
 BSL6D_API int bsl6d_advect_pointwise(bsl6d_ctx* ctx, const double* f_in, double* f_out, int dim,
                            const double* alpha_cells, int q, void* stream);
 

@@ -1117,6 +1117,10 @@ int bsl6d_advect_pointwise(bsl6d_ctx* c, const double* f_in, double* f_out, int 
     a.alpha = alpha_cells;
     a.inner = (uint32_t)inner;
     a.outer = (uint32_t)outer;
+    a.n = (uint32_t)n[dim];
+    a.periodic = is_periodic(c, dim) ? 1u : 0u;
+    a.pb = (uint32_t)pc.unit;
+    a.ld = (uint32_t)(n[dim] | 1);
     unsigned grid;
     if (pc.unit) {
         grid = (unsigned)((outer + (size_t)pc.unit - 1) / (size_t)pc.unit);

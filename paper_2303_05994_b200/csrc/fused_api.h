@@ -63,6 +63,7 @@ struct PointwiseChoice {
     int threads;
     size_t smem;
     int unit;              // > 0: unit-stride kernel, a block takes this many pencils
+    int generic;           // run-time-extent kernel: PointwiseArgs::n / periodic / pb / ld are read
 };
 bool pointwise_lookup(int n, int q, bool periodic, bool unit_stride, PointwiseChoice& out);
 }  // namespace bsl6d
