@@ -67,6 +67,8 @@ struct KernelChoice {
     size_t smem;
     int kind;                 // 0 strided, 1 unit, 2 generic
     int gen_T;                // generic: threads; unit and strided: segments per pencil S
+    sweep_fn fn_oop;          // strided only, may be null: the kernel for f_in != f_out (sweep_stream_kernel)
+    int oop_threads;
 };
 
 // Launch shape of the strided sweep: T threads per block, at least MINB resident blocks per SM (caps the
@@ -111,7 +113,16 @@ KernelChoice strided_choice() {
 #else
     constexpr int MINB = S == 1 ? strided_minblocks<N, Q, P>() : 4;
 #endif
-    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S};
+    // Out of place, long periodic pencils stream through a register window instead (sweep_stream_kernel: 96-122 instead
+    // of 162-168 registers at N = 48, Q = 10; C5 x sweeps +1.7-2.8 % in alternating runs on one box).  Zero-extended
+    // long pencils (N = 64, Q = 6) and the pencils that fit 128 registers anyway measured 0.6-2 % slower that way.
+    if constexpr (P && S == 1 && strided_regs_wanted<N, Q, P>() > 128) {
+        KernelChoice kc{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S};
+        kc.fn_oop = bsl6d::sweep_stream_kernel<N, Q, P, 128, 4, 12>;
+        kc.oop_threads = 128;
+        return kc;
+    }
+    return KernelChoice{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S, nullptr, 0};
 }
 
 // Launch shape of the unit-stride sweep: S segments per pencil, T threads (a multiple of 32*S), MINB blocks/SM.
@@ -129,7 +140,7 @@ KernelChoice unit_choice() {
     constexpr int S = unit_segments<N, Q>();
     constexpr int T = unit_threads<N, Q>();
     constexpr int MINB = unit_minblocks<N, Q>();
-    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N | 1), 1, S};
+    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N | 1), 1, S, nullptr, 0};
 }
 
 template <int N, bool P>
@@ -227,7 +238,7 @@ int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     if (per_thread * T > cap) return BSL6D_EUNSUPPORTED;
     // gen_T = pencils per block; the unit-stride fallback runs kGenericUnitSegments threads per pencil
     const bool unit = inner == 1 && !periodic;
-    k = KernelChoice{nullptr, unit ? T * kGenericUnitSegments : T, per_thread * T, 2, T};
+    k = KernelChoice{nullptr, unit ? T * kGenericUnitSegments : T, per_thread * T, 2, T, nullptr, 0};
     return BSL6D_OK;
 }
 
@@ -321,6 +332,10 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     if (rc) return rc;
     rc = choose_kernel(c, dim, kc);
     if (rc) return rc;
+    if (kc.fn_oop && f_in != f_out) {                      // out of place: the streaming variant where there is one
+        kc.fn = kc.fn_oop;
+        kc.threads = kc.oop_threads;
+    }
 
     SweepArgs a;
     std::memset(&a, 0, sizeof(a));

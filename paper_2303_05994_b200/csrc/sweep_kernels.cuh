@@ -198,6 +198,75 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
     }
 }
 
+// ---- a4, out of place: the same sweep with the pencil STREAMED through a register window --------------------
+// Only for f_in != f_out (an output row may be stored before the input rows behind it have been read).  A thread still
+// owns a pencil, but holds Q-1+D+1 of its values at a time instead of all N: row t (in shifted order) is loaded D
+// outputs before the first output that needs it, the stores in between keep the loads where they are written.  For
+// long pencils with wide stencils (N = 48, Q = 10: 162-168 registers, 12 warps per SM in sweep_strided_kernel) this
+// roughly halves the registers.  Periodic pencils keep their first Q-1 rows for the wrap at the end.  Arithmetic and
+// its order are those of sweep_strided_kernel: bit-identical results.
+template <int N, int Q, bool PERIODIC, int T, int MINB, int D>
+__global__ void __launch_bounds__(T, MINB) sweep_stream_kernel(const SweepArgs a) {
+    const uint32_t tp = threadIdx.x;
+    uint32_t i, o;
+    bool live;
+    if (a.ti_log2 == kFlatPencils) {
+        const uint32_t p = blockIdx.x * T + tp;
+        live = p < a.nib;
+        o = p / a.inner;
+        i = p - o * a.inner;
+    } else {
+        const uint32_t ti_mask = (1u << a.ti_log2) - 1u;
+        const uint32_t bo = blockIdx.x / a.nib;
+        const uint32_t bi = blockIdx.x - bo * a.nib;
+        i = (bi << a.ti_log2) + (tp & ti_mask);
+        o = bo * (T >> a.ti_log2) + (tp >> a.ti_log2);
+        live = i < a.inner && o < a.outer;
+    }
+    if (!live) return;
+    long long k;
+    double theta;
+    split_shift(__ldg(a.src + src_offset(a.terms, o, i)), a.scale, k, theta);
+    const size_t stride = a.inner;
+    const size_t base = (size_t)o * N * stride + i;
+    const double* pin = a.in + base;
+    double* pout = a.out + base;
+    int r0;
+    if (PERIODIC) {
+        r0 = (int)((k + (long long)(1 - Q / 2)) % (long long)N);
+        if (r0 < 0) r0 += N;
+    } else {
+        long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
+        kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
+        r0 = (int)kc + (1 - Q / 2);
+    }
+    auto load_row = [&](int t) -> double {                 // shifted row t = 0 .. N+Q-2
+        int row = r0 + t;
+        if (PERIODIC) {
+            if (row >= N) row -= N;
+            return BSL6D_LD(pin + (size_t)row * stride);
+        }
+        return (row >= 0 && row < N) ? BSL6D_LD(pin + (size_t)row * stride) : 0.0;
+    };
+    // u[t], t = 0 .. N+Q-2: fully unrolled, each element lives from its load to its last use; periodic: u[N+t] is u[t]
+    constexpr int NU = N + Q - 1;
+    constexpr int NL = PERIODIC ? N : NU;                  // rows that are loaded
+    double u[NU];
+#pragma unroll
+    for (int t = 0; t < NL && t < Q - 1 + D; ++t) u[t] = load_row(t);
+    double w[Q];
+    lagrange_weights<Q>(theta, w);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        const int tl = j + Q - 1 + D;
+        if (tl < NL) u[tl] = load_row(tl);
+        double acc = w[0] * u[(PERIODIC && j >= N) ? j - N : j];
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[(PERIODIC && j + m >= N) ? j + m - N : j + m], acc);
+        BSL6D_ST(pout + (size_t)j * stride, acc);
+    }
+}
+
 // ---- a3: unit-stride sweep (swept dim is the contiguous one; always a v dim => zero extension) -------------
 // A block owns PB = T/S consecutive pencils = one contiguous chunk of PB*N doubles.  Coalesced load -> padded
 // smem (row stride N+1 doubles: conflict-free for "lane = pencil" access).  A pencil is cut into S segments of
@@ -295,8 +364,13 @@ __global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int
     const size_t stride = a.inner;
     const size_t base = (size_t)o * n * stride + i;
     double* col = tile + threadIdx.x;
-#pragma unroll 8
-    for (int r = 0; r < n; ++r) col[r * T] = __ldcs(a.in + base + (size_t)r * stride);
+    {   // 8-byte asynchronous copies: all n rows of the column in flight, nothing staged in registers
+        const uint32_t dcol = (uint32_t)__cvta_generic_to_shared(col);
+        const double* src = a.in + base;
+        for (int r = 0; r < n; ++r)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dcol + (uint32_t)(r * T * 8)), "l"(src + (size_t)r * stride) : "memory");
+        asm volatile("cp.async.wait_all;" ::: "memory");       // a thread reads only what it copied itself
+    }
 
     double w[Q];
     lagrange_weights<Q>(theta, w);
@@ -358,7 +432,11 @@ __global__ void __launch_bounds__(PB * S) sweep_generic_unit_kernel(const SweepA
     const uint32_t nelem = np * (uint32_t)n;
     const double* pin = a.in + p0 * n;
     double* pout = a.out + p0 * n;
-    for (uint32_t e = threadIdx.x; e < nelem; e += T) tin[(e / n) * LD + (e % n)] = __ldcs(pin + e);
+    for (uint32_t e = threadIdx.x; e < nelem; e += T) {
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tin + (e / n) * LD + (e % n));
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(pin + e) : "memory");
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
     const uint32_t pl = threadIdx.x % PB;
     const int seg = (int)(threadIdx.x / PB);

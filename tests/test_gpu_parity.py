@@ -120,6 +120,9 @@ GRIDS = [
     ((37, 2, 2, 37, 2, 37), 7),       # strided<37,8> periodic + zero with flattened pencil indexing, unit<37,8>
     ((3, 37, 37, 37, 37, 37), 9),     # strided<37,10> on inner extents 37^k (no multiple of the warp width), unit<37,10>
     ((36, 3, 2, 36, 2, 36), 5),       # extent 36: no specialised instance -> generic strided + generic unit, q = 6
+    ((64, 2, 48, 4, 4, 8), 9),        # long periodic pencils: out of place = sweep_stream_kernel<64,10>, <48,10>; in place = strided
+    ((48, 3, 5, 2, 3, 7), 5),         # sweep_stream_kernel<48,6> with a ragged inner extent (flattened pencil index)
+    ((5, 64, 3, 3, 1, 2), 3),         # sweep_stream_kernel<64,4>, inner = 18
 ]
 
 
