@@ -14,14 +14,18 @@
 // pipe and the shared-memory pipe overlap instead of taking turns (the round-1 kernels ran 2 lock-stepped blocks per
 // SM: load, then compute, then store).
 // The shared-memory tile is dense (a TMA box cannot be padded): sweeps along a are bank-conflict free, sweeps along b
-// see 2-way conflicts on their shared-memory accesses (two rows 2 KB apart per half-warp); measured cheaper than
-// any layout that needs a second pass through shared memory.
+// would see 2-way conflicts (two rows 2 KB apart per half-warp); pencil_in_place's `rot` removes them without a second
+// pass through shared memory by letting the odd rows run one element ahead.
 // Per sweep the arithmetic (split_shift, lagrange_weights, the fma chain) is that of sweep_kernels.cuh, so a pass is
 // bit-identical to the same sweeps launched one by one.
 #pragma once
 #include <cuda.h>
 
 #include "sweep_kernels.cuh"
+
+#ifndef BSL6D_PTILE_ROT
+#define BSL6D_PTILE_ROT 1
+#endif
 
 namespace bsl6d {
 
@@ -93,16 +97,34 @@ __device__ __forceinline__ void group_sync(int id, int count) {
 
 // One pencil of N points at shared-memory address `base`, element j at base + j*STRIDE bytes: in place.
 // Loads in shifted order (all before the first store), weights, FMA chains: the arithmetic of sweep_strided_kernel.
+//
+// rot (0 or 1) turns the order in which the thread touches its pencil by one element: with rot = 1 the t-th load
+// instruction reads the element AFTER the one a rot = 0 thread reads, and the j-th store writes output j+1.  The
+// values are the same; only which instruction moves which element changes.  Sweeps along b pass par = i_a & 1 and get
+// rot = (r0 + par) & 1, so that the row a thread touches at instruction t has the parity of i_a + t whatever its
+// displacement: the two pencils of a half-warp there lie a whole plane (a multiple of 128 bytes) apart, i.e. in the
+// same banks when they touch the same row, and the turn keeps them one 64-byte tile row -- half the banks -- apart.
+// The dense tile a TMA box writes is then swept without bank conflicts in both directions (ncu, C2 v1+v2: 1.7e8
+// conflict wavefronts of 4.6e8 before).  Periodic pencils: a cyclic turn of the N registers.  Zero-extended pencils
+// hold N+Q-1 values u[t] = in[r0 + (t + rot) mod NU]; outputs j+rot come out of registers j..j+Q-1 for j < N-1, and the
+// one output left (N-1 for rot = 0, 0 for rot = 1) out of a register set picked by rot.  par < 0: no turn.
+// Measured (alternating runs on one box, ms per pass): v1+v2 2.90 -> 2.75 at C2, 11.34 -> 11.08 at C5 -- the passes are
+// bound by dependent latency at 16 warps per SM more than by the shared-memory pipe; x3+v1 (a periodic) got SLOWER with
+// the turn (3.03 -> 3.56 at C2, unexplained), so it is applied only when a is zero-extended.
 template <int N, int Q, bool PERIODIC, uint32_t STRIDE>
-__device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, double scale) {
+__device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, double scale, int par = -1) {
     long long k;
     double theta;
     split_shift(sval, scale, k, theta);
     constexpr int NU = PERIODIC ? N : N + Q - 1;
     double u[NU];
+    int rot;
     if (PERIODIC) {
         int r0 = (int)((k + (long long)(1 - Q / 2)) % (long long)N);
         if (r0 < 0) r0 += N;
+        rot = par < 0 ? 0 : ((r0 + par) & 1);
+        r0 += rot;
+        if (r0 >= N) r0 -= N;
 #pragma unroll
         for (int t = 0; t < N; ++t) {
             int row = r0 + t;
@@ -113,9 +135,12 @@ __device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, doub
         long long kc = k < -(long long)(2 * N + 2 * Q) ? -(long long)(2 * N + 2 * Q) : k;
         kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
         const int r0 = (int)kc + (1 - Q / 2);
+        rot = par < 0 ? 0 : ((r0 + par) & 1);
 #pragma unroll
         for (int t = 0; t < NU; ++t) {
-            const int row = r0 + t;
+            int tt = t + rot;
+            if (tt >= NU) tt -= NU;
+            const int row = r0 + tt;
             double v = 0.0;
             if (row >= 0 && row < N) v = lds_f64(base + (uint32_t)row * STRIDE);
             u[t] = v;
@@ -123,12 +148,29 @@ __device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, doub
     }
     double w[Q];
     lagrange_weights<Q>(theta, w);
+    if (PERIODIC) {
 #pragma unroll
-    for (int j = 0; j < N; ++j) {
-        double acc = w[0] * u[PERIODIC ? (j % N) : j];
+        for (int j = 0; j < N; ++j) {
+            double acc = w[0] * u[j % N];
 #pragma unroll
-        for (int m = 1; m < Q; ++m) acc = fma(w[m], u[PERIODIC ? ((j + m) % N) : (j + m)], acc);
-        sts_f64(base + (uint32_t)j * STRIDE, acc);
+            for (int m = 1; m < Q; ++m) acc = fma(w[m], u[(j + m) % N], acc);
+            int jo = j + rot;
+            if (jo >= N) jo -= N;
+            sts_f64(base + (uint32_t)jo * STRIDE, acc);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < N - 1; ++j) {
+            double acc = w[0] * u[j];
+#pragma unroll
+            for (int m = 1; m < Q; ++m) acc = fma(w[m], u[j + m], acc);
+            sts_f64(base + (uint32_t)(j + rot) * STRIDE, acc);
+        }
+        // the output left: N-1 from in[r0+N-1+m] = u[N-1+m] (rot = 0), or 0 from in[r0+m] = u[m-1], u[NU-1] for m = 0 (rot = 1)
+        double acc = w[0] * (rot ? u[NU - 1] : u[N - 1]);
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(w[m], rot ? u[m - 1] : u[N - 1 + m], acc);
+        sts_f64(base + (uint32_t)(rot ? 0 : N - 1) * STRIDE, acc);
     }
 }
 
@@ -228,7 +270,7 @@ __global__ void __launch_bounds__((PTileGeom<NA, NB>::THREADS), 1)
                 for (int p = gt; p < NA * C; p += GT) {
                     const uint32_t ia = (uint32_t)p / C, c = (uint32_t)p % C;
                     const double sval = p == gt ? sval_first : shift_source(s, p);
-                    pt::pencil_in_place<NB, Q, PB, (uint32_t)ROW>(buf + ia * (uint32_t)PLANE + c * 8u, sval, sw.scale);
+                    pt::pencil_in_place<NB, Q, PB, (uint32_t)ROW>(buf + ia * (uint32_t)PLANE + c * 8u, sval, sw.scale, (BSL6D_PTILE_ROT && !PA) ? (int)(ia & 1u) : -1);
                 }
             }
             pt::group_sync(1 + g, GT);
