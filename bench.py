@@ -415,7 +415,7 @@ def measure_workload(G: Gpu, w, K: int, W: int, want_fused: bool, sample_clocks:
             per_dim[nm]["Gpoint-updates/s"] = nl * npts / (per_op[nm] * 1e-3) / 1e9
     traffic, traffic_src = read_traffic(w.name)
     roofline = {"bound": "hbm",
-                "kernel": f"sweep_strided_kernel ({n_strided} of {launches // K} launches per step)",
+                "kernel": f"strided sweep family: sweep_strided_kernel / sweep_stream_kernel ({n_strided} of {launches // K} launches per step)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "frac_of_8TBs_spec": achieved / 8000.0, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": 16 * npts, "avg_launch_ms": strided_ms,

@@ -204,7 +204,9 @@ BSL6D_API int bsl6d_run_host(bsl6d_ctx* ctx, const double* f_in_host, double* f_
 BSL6D_API const char* bsl6d_strerror(int code);
 BSL6D_API int bsl6d_last_cuda_error(const bsl6d_ctx* ctx);          /* cudaError_t of the last BSL6D_ECUDA, else 0 */
 BSL6D_API long long bsl6d_launch_count(const bsl6d_ctx* ctx);       /* kernels launched by this context so far */
-/* Name of the kernel variant bsl6d_advect* would launch for `dim` ("strided<N,Q>", "unit<N,Q>", "generic"). */
+/* Name of the kernel variant bsl6d_advect* would launch for `dim` ("strided<N,Q,..>", "unit<N,Q,..>", "generic<..>";
+ * "stream<N,Q,..> (in place: strided<..>)" where an out-of-place sweep streams its pencils through a register window
+ * and the in-place sweep holds them whole -- bit-identical results either way). */
 BSL6D_API int bsl6d_kernel_name(const bsl6d_ctx* ctx, int dim, char* buf, int buflen);
 BSL6D_API int bsl6d_version(void);
 

@@ -1002,6 +1002,9 @@ int bsl6d_kernel_name(const bsl6d_ctx* c, int dim, char* buf, int buflen) {
     else if (k.kind == 0 && k.gen_T > 1)
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,S=%d,T=%d>", kind, (int)c->g.n[dim], c->q,
                       is_periodic(c, dim) ? "periodic" : "zero", k.gen_T, k.threads);
+    else if (k.kind == 0 && k.fn_oop)                         // f_in != f_out runs the streaming variant
+        std::snprintf(buf, (size_t)buflen, "stream<N=%d,Q=%d,%s,T=%d> (in place: strided<T=%d>)", (int)c->g.n[dim], c->q,
+                      is_periodic(c, dim) ? "periodic" : "zero", k.oop_threads, k.threads);
     else
         std::snprintf(buf, (size_t)buflen, "%s<N=%d,Q=%d,%s,T=%d>", kind, (int)c->g.n[dim], c->q,
                       is_periodic(c, dim) ? "periodic" : "zero", k.threads);
