@@ -131,7 +131,15 @@ template <int N, int Q> constexpr int unit_segments() { return (N % BSL6D_TUNE_U
 template <int N, int Q> constexpr int unit_minblocks() { return BSL6D_TUNE_UMINB; }
 #else
 template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 4 : 1; }
-template <int N, int Q> constexpr int unit_minblocks() { return 4; }
+template <int N, int Q> constexpr int unit_minblocks() { return N >= 48 ? 6 : 4; }
+#endif
+// Tile filled by cp.async (true) or by loads staged in registers.  Alternating runs on one box, v3 sweep in-step, GB/s:
+// C3 (N = 64, q = 6, with 6 blocks/SM) 6440-6486 -> 6915-6948; C2 (N = 32, q = 8) 6631-6668 -> 6946-7009;
+// C5 (N = 32, q = 10) 6715 -> 6600-6612, so the widest stencil on short pencils keeps the register fill.
+#ifdef BSL6D_TUNE_UASYNC
+template <int N, int Q> constexpr bool unit_async() { return BSL6D_TUNE_UASYNC != 0; }
+#else
+template <int N, int Q> constexpr bool unit_async() { return unit_segments<N, Q>() > 1 || Q <= 8; }
 #endif
 template <int N, int Q> constexpr int unit_threads() { return 128 % (32 * unit_segments<N, Q>()) == 0 ? 128 : 32 * unit_segments<N, Q>(); }
 
@@ -140,7 +148,7 @@ KernelChoice unit_choice() {
     constexpr int S = unit_segments<N, Q>();
     constexpr int T = unit_threads<N, Q>();
     constexpr int MINB = unit_minblocks<N, Q>();
-    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB>, T, sizeof(double) * (T / S) * (N | 1), 1, S, nullptr, 0};
+    return KernelChoice{bsl6d::sweep_unit_kernel<N, Q, S, T, MINB, unit_async<N, Q>()>, T, sizeof(double) * (T / S) * (N | 1), 1, S, nullptr, 0};
 }
 
 template <int N, bool P>

@@ -109,8 +109,10 @@ __device__ __forceinline__ void group_sync(int id, int count) {
 // hold N+Q-1 values u[t] = in[r0 + (t + rot) mod NU]; outputs j+rot come out of registers j..j+Q-1 for j < N-1, and the
 // one output left (N-1 for rot = 0, 0 for rot = 1) out of a register set picked by rot.  par < 0: no turn.
 // Measured (alternating runs on one box, ms per pass): v1+v2 2.90 -> 2.75 at C2, 11.34 -> 11.08 at C5 -- the passes are
-// bound by dependent latency at 16 warps per SM more than by the shared-memory pipe; x3+v1 (a periodic) got SLOWER with
-// the turn (3.03 -> 3.56 at C2, unexplained), so it is applied only when a is zero-extended.
+// bound by dependent latency at 16 warps per SM more than by the shared-memory pipe.  For x3+v1 (a periodic) no gain
+// could be shown (C2: 3.03 without, 3.56 with the turn in one pair of runs, but the same kernel without the turn also
+// measured 3.95 on another box: that pass varies more from run to run than the turn could win), so the turn is applied
+// only where a is zero-extended.
 template <int N, int Q, bool PERIODIC, uint32_t STRIDE>
 __device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, double scale, int par = -1) {
     long long k;
