@@ -113,7 +113,8 @@ BSL6D_API int bsl6d_strang_step(bsl6d_ctx* ctx, double* f, double* f_tmp, const 
  * as single sweeps, and so does a PAIR that measurement says does not pay (row segments under 64 bytes, or a tile
  * whose rows lie >= 64 MB apart).  The planner picks the grouping with the fewest passes.
  * bsl6d_set_fusion(ctx, 0) turns grouping off (every sweep its own pass), 1 is the default policy, 2 fuses
- * wherever a kernel exists (for tests and tuning); returns the old setting. */
+ * wherever a kernel exists; for tests and tuning also 3 (round-1 tile kernels only), 4 (those + whole-v-block
+ * passes), 5 (the default policy without whole-v-block passes); returns the old setting. */
 typedef struct bsl6d_sweep {
     int32_t dim;             /* swept dim 0..5 */
     uint32_t src_dim_mask;   /* dims the shift source is dense over (bit d), must not contain `dim` */

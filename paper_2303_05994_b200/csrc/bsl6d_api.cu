@@ -545,7 +545,7 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
     // (C2: q = 8, C5: q = 10, in-step medians); they only have to rank the alternatives:
     //   single sweep                      1
     //   persistent tile pass, n sweeps    0.45 + (0.035 q + 0.07) n      (+0.3 when an extent exceeds 32: two buffers)
-    //   v-block pass, n sweeps            0.90 + (0.020 q + 0.03) n      (+1.3 per switch between v1/v2 sweeps and v3
+    //   v-block pass, n sweeps            1.10 + (0.020 q + 0.03) n      (+1.3 per switch between v1/v2 sweeps and v3
     //                                                                      sweeps: the block is re-tiled through L2)
     //   round-1 tile kernels              pair 0.7 + 0.10 q,  a-b-a triple 0.7 + 0.13 q
     // Fusion mode 2 ("wherever a kernel exists") counts passes instead: every pass costs 1, ties go to the larger group.
@@ -590,7 +590,7 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
                 if (len < c->vblock_min) continue;
                 Pass p;
                 if (!try_vblock(c, sw, i, len, p)) break;
-                const double cost = by_count ? 1.0 : 0.90 + (0.020 * q + 0.03) * len + 1.3 * switches;
+                const double cost = by_count ? 1.0 : 1.10 + (0.020 * q + 0.03) * len + 1.3 * switches;
                 const double total = cost + best[i + len];
                 if (better(total, best[i])) { best[i] = total; pick[i] = -len; candv[i] = p; }
             }
@@ -1111,13 +1111,13 @@ int bsl6d_set_boundary(bsl6d_ctx* c, int dim, int open) {
 
 int bsl6d_set_fusion(bsl6d_ctx* c, int enable) {
     if (!c) return BSL6D_EINVAL;
-    if (enable < 0 || enable > 4) return BSL6D_EINVAL;
+    if (enable < 0 || enable > 5) return BSL6D_EINVAL;
     const int old = c->fusion_mode;
     c->fusion_mode = enable;
     c->fusion = enable ? 1 : 0;
     c->fuse_all = enable == 2 ? 1 : 0;
-    c->use_ptile = (enable == 1 || enable == 2) ? 1 : 0;      // 3: round-1 tile kernels only; 4: those + v-block passes
-    c->use_vblock = enable == 3 ? 0 : 1;
+    c->use_ptile = (enable == 1 || enable == 2 || enable == 5) ? 1 : 0;   // 3: round-1 tile kernels only; 4: those + v-block passes
+    c->use_vblock = (enable == 3 || enable == 5) ? 0 : 1;               // 5: planner without v-block passes
     c->use_fused = 1;
     return old;
 }

@@ -264,7 +264,7 @@ def test_random_chains_every_planner_mode_equals_single_sweeps(n, degree, seed):
             chain = [(d, torch.from_numpy(np.ascontiguousarray(s)).cuda(), m, sc) for d, s, m, sc in chain_host]
             ctx.set_fusion(0)
             single = ctx.advect_seq(fd, torch.empty_like(fd), chain)
-            for mode in (1, 2, 3, 4):
+            for mode in (1, 2, 3, 4, 5):
                 ctx.set_fusion(mode)
                 npass = ctx.seq_passes(chain)
                 assert 1 <= npass <= ns
