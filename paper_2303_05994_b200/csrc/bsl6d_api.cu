@@ -116,7 +116,10 @@ KernelChoice strided_choice() {
     // Out of place, long periodic pencils stream through a register window instead (sweep_stream_kernel: 96-122 instead
     // of 162-168 registers at N = 48, Q = 10; C5 x sweeps +1.7-2.8 % in alternating runs on one box).  Zero-extended
     // long pencils (N = 64, Q = 6) and the pencils that fit 128 registers anyway measured 0.6-2 % slower that way.
-    if constexpr (P && S == 1 && strided_regs_wanted<N, Q, P>() > 128) {
+#ifndef BSL6D_TUNE_STREAM_REGS
+#define BSL6D_TUNE_STREAM_REGS 128
+#endif
+    if constexpr (P && S == 1 && strided_regs_wanted<N, Q, P>() > BSL6D_TUNE_STREAM_REGS) {
         KernelChoice kc{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S};
         kc.fn_oop = bsl6d::sweep_stream_kernel<N, Q, P, 128, 4, 12>;
         kc.oop_threads = 128;
