@@ -592,7 +592,8 @@ def run_ours(args, w, extra):
     K, W = args.steps, args.warmup
     want_e2e = not args.no_e2e
     e2e_w = w
-    if want_e2e and not host_memory_allows(8 * w.npts):
+    # every rank of the node pins its own copy: the box must hold `world` of them, and all ranks must decide alike
+    if want_e2e and max_over_ranks(0.0 if host_memory_allows(8 * w.npts * G.world) else 1.0, G.dev) != 0.0:
         import bsl6d_workloads as wl
         e2e_w = wl.C2                                     # not enough host memory to pin this workload's f
     rec, f0_host = measure_workload(G, w, K, W, not args.no_fused, True, want_e2e and e2e_w is w)
