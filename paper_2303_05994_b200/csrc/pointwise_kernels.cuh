@@ -9,8 +9,8 @@
 // is a compile-time constant in the kernels compiled per extent.
 //
 // Round 2 (second half): (i) the per-point evaluation uses the symmetry of the centred equidistant nodes
-// (interp_odd below: 4h + 5 + 8h... about 4q fp64 instructions instead of 6q for q separate weights), because widths
-// 7 and 9 were co-limited by the fp64 pipe; (ii) the strided kernel no longer holds the displacements of a whole
+// (interp_odd below: about 4.5q fp64 instructions instead of 6q for q separate weights -- 41 against 52 at q = 9),
+// because widths 7 and 9 were co-limited by the fp64 pipe; (ii) the strided kernel no longer holds the displacements of a whole
 // pencil in registers: f and alpha stream through a look-ahead of D rows (loads issued D outputs ahead of their
 // use, stores in between), which halves the registers and doubles the resident warps; (iii) run-time-extent kernels
 // (pointwise_generic_kernel, pointwise_generic_unit_kernel) serve every extent without a compiled instance.
@@ -23,18 +23,17 @@
 
 namespace bsl6d {
 
-// c[m] = 1 / prod_{j != m, |j| <= H} (m - j) for m = 0..H (c[-m] == c[m]: q - 1 is even), mc[m] = m * c[m]
+// c[m] = 1 / prod_{j != m, |j| <= H} (m - j) for m = 0..H (c[-m] == c[m]: q - 1 is even)
 template <int Q>
 struct OddSym {
-    double c[(Q + 1) / 2], mc[(Q + 1) / 2];
-    constexpr OddSym() : c(), mc() {
+    double c[(Q + 1) / 2];
+    constexpr OddSym() : c() {
         constexpr int H = (Q - 1) / 2;
         for (int m = 0; m <= H; ++m) {
             double d = 1.0;
             for (int j = -H; j <= H; ++j)
                 if (j != m) d *= (double)(m - j);
             c[m] = 1.0 / d;
-            mc[m] = (double)m / d;
         }
     }
 };
