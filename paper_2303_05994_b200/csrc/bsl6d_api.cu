@@ -134,7 +134,7 @@ template <int N, int Q> constexpr int unit_segments() { return (N % BSL6D_TUNE_U
 template <int N, int Q> constexpr int unit_minblocks() { return BSL6D_TUNE_UMINB; }
 #else
 template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 4 : 1; }
-template <int N, int Q> constexpr int unit_minblocks() { return N >= 48 ? 6 : 4; }
+template <int N, int Q> constexpr int unit_minblocks() { return (N >= 48 && Q <= 8) ? 6 : 4; }   // q = 10 at 80 registers spills
 #endif
 // Tile filled by cp.async (true) or by loads staged in registers.  Alternating runs on one box, v3 sweep in-step, GB/s:
 // C3 (N = 64, q = 6, with 6 blocks/SM) 6440-6486 -> 6915-6948; C2 (N = 32, q = 8) 6631-6668 -> 6946-7009;
