@@ -536,8 +536,8 @@ def measure_workload(G: Gpu, w, K: int, W: int, want_fused: bool, sample_clocks:
     return rec, f0_host
 
 
-def host_memory_allows(nbytes: int) -> bool:
-    """Is it safe to pin `nbytes` of host memory on this box (physical memory and cgroup limit)?"""
+def host_memory_allows(nbytes: int, factor: float = 2.5) -> bool:
+    """Is it safe to pin `nbytes` more of host memory on this box (physical memory and cgroup limit)?"""
     try:
         import psutil
         avail = psutil.virtual_memory().available
@@ -551,24 +551,34 @@ def host_memory_allows(nbytes: int) -> bool:
                 avail = min(avail, int(s))
         except Exception:
             pass
-    return avail >= 2.5 * nbytes
+    return avail >= factor * nbytes
 
 
 def measure_e2e(G: Gpu, w, f0_host, K: int):
-    """The same step through bsl6d_run_host on HOST buffers (pinned), copies inside the timed region."""
+    """The same step through the host-buffer entry points (pinned HOST buffers), copies inside the timed region.
+    Two legs: `serial` = bsl6d_run_host, one step after the other (upload, ops, download); `value` = the same steps
+    through bsl6d_run_host_begin / _end with two steps in flight, so that the upload of step k+1 overlaps the download
+    of step k (every step still uploads its own input and downloads its own result; the host link is full duplex).
+    The pipelined leg needs one more pinned buffer of the size of f; without the memory for it the serial figure is
+    reported as `value`."""
     torch, bsl = G.torch, G.bsl
     nx = w.n[0] * w.n[1] * w.n[2]
-    E_host = [torch.from_numpy(e) for e in w.E()]
-    hops, n_small = [], 0
-    for name, kind, dim, dt, B in step_ops(w):
-        if kind == "advect":
-            hops.append({"kind": "advect", "dim": dim, "dt": dt,
-                         "shift_source": None if dim < 3 else E_host[dim - 3]})
-            n_small += 0 if dim < 3 else nx
-        elif kind == "rotate":
-            hops.append({"kind": "rotate", "B": B, "dt": dt})
-        else:
-            hops.append({"kind": "density", "rho_host": torch.empty(w.n[:3], dtype=torch.float64, pin_memory=True)})
+    E_host = [torch.from_numpy(e).pin_memory() for e in w.E()]
+
+    def make_ops():
+        hops, n_small = [], 0
+        for name, kind, dim, dt, B in step_ops(w):
+            if kind == "advect":
+                hops.append({"kind": "advect", "dim": dim, "dt": dt,
+                             "shift_source": None if dim < 3 else E_host[dim - 3]})
+                n_small += 0 if dim < 3 else nx
+            elif kind == "rotate":
+                hops.append({"kind": "rotate", "B": B, "dt": dt})
+            else:
+                hops.append({"kind": "density", "rho_host": torch.empty(w.n[:3], dtype=torch.float64, pin_memory=True)})
+        return hops, n_small
+
+    hops, n_small = make_ops()
     ctx = bsl.create(w.n, w.lo, w.dx, w.degree)
     ctx.set_fusion(0)
     ke = max(1, min(K, 5 if w.npts < (1 << 31) else 2))
@@ -579,11 +589,41 @@ def measure_e2e(G: Gpu, w, f0_host, K: int):
         ctx.run_host(f0_host, f0_host, hops)
     torch.cuda.synchronize()
     te = max_over_ranks(time.perf_counter() - t0, G.dev)
+    serial = {"value": whole_job_value(w.npts, n_sweeps(w), ke, G.world, 1e3 * te), "steps": ke,
+              "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (one step after the other)"}
+    rec = {"value": serial["value"], "unit": UNIT,
+           "h2d_bytes_per_step": 8 * w.npts + 8 * n_small, "d2h_bytes_per_step": 8 * w.npts + 8 * nx,
+           "steps": ke, "ms_per_step": serial["ms_per_step"], "api": "bsl6d_run_host (pinned host buffers)",
+           "workload": workload_label(w)}
+    # ---- two steps in flight: both slots upload f0_host (read only here), each downloads into a buffer of its own ----
+    free_dev = torch.cuda.mem_get_info()[0]
+    ok = host_memory_allows(2 * 8 * w.npts * G.world, factor=1.5) and free_dev > 1.2 * 8 * w.npts
+    if max_over_ranks(0.0 if ok else 1.0, G.dev) == 0.0:
+        outs = [torch.empty(w.n, dtype=torch.float64, pin_memory=True) for _ in range(2)]
+        hops2 = [hops, make_ops()[0]]
+        kp = max(4, 2 * ke)
+        for sl in (0, 1):                                     # warm-up: allocates the second slot's device buffer
+            ctx.run_host_begin(f0_host, outs[sl], hops2[sl], sl)
+        ctx.run_host_end(0)
+        ctx.run_host_end(1)
+        G.barrier()
+        t0 = time.perf_counter()
+        for k in range(kp):
+            sl = k & 1
+            if k >= 2:
+                ctx.run_host_end(sl)                          # the step that used this slot's buffers is complete
+            ctx.run_host_begin(f0_host, outs[sl], hops2[sl], sl)
+        ctx.run_host_end(0)
+        ctx.run_host_end(1)
+        tp = max_over_ranks(time.perf_counter() - t0, G.dev)
+        rec.update({"value": whole_job_value(w.npts, n_sweeps(w), kp, G.world, 1e3 * tp), "steps": kp,
+                    "ms_per_step": 1e3 * tp / kp,
+                    "api": "bsl6d_run_host_begin / bsl6d_run_host_end, two steps in flight (pinned host buffers): "
+                           "the upload of step k+1 overlaps the download of step k",
+                    "serial": serial})
+        del outs
     ctx.destroy()
-    return {"value": whole_job_value(w.npts, n_sweeps(w), ke, G.world, 1e3 * te), "unit": UNIT,
-            "h2d_bytes_per_step": 8 * w.npts + 8 * n_small, "d2h_bytes_per_step": 8 * w.npts + 8 * nx,
-            "steps": ke, "ms_per_step": 1e3 * te / ke, "api": "bsl6d_run_host (pinned host buffers)",
-            "workload": workload_label(w)}
+    return rec
 
 
 def run_ours(args, w, extra):

@@ -200,6 +200,17 @@ typedef struct bsl6d_host_op {
 } bsl6d_host_op;
 BSL6D_API int bsl6d_run_host(bsl6d_ctx* ctx, const double* f_in_host, double* f_out_host,
                    const bsl6d_host_op* ops, int nops);
+/* The same in two halves, so that two independent problems can be in flight at once: bsl6d_run_host_begin enqueues
+ * upload, ops and download on the internal stream of `slot` (0 or 1; each slot has its own device buffers) and returns
+ * without waiting; bsl6d_run_host_end(ctx, slot) waits for everything begun on that slot.  With two slots the upload
+ * of one problem overlaps the download of the other (the host link is full duplex) and the kernels of either -- for a
+ * stream of problems the step time drops from upload + compute + download to about max(upload, download).  Until
+ * bsl6d_run_host_end returns, f_in_host, f_out_host, every shift_source and rho_host of the call must stay valid and
+ * untouched (the ops array itself is consumed before _begin returns).  A second _begin on a slot queues behind the
+ * first.  bsl6d_run_host(...) == _begin(..., 0) followed by _end(ctx, 0). */
+BSL6D_API int bsl6d_run_host_begin(bsl6d_ctx* ctx, const double* f_in_host, double* f_out_host,
+                         const bsl6d_host_op* ops, int nops, int slot);
+BSL6D_API int bsl6d_run_host_end(bsl6d_ctx* ctx, int slot);
 
 /* ---- introspection ------------------------------------------------------------------------------------ */
 BSL6D_API const char* bsl6d_strerror(int code);

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libbsl6d.so")
 #: every symbol include/bsl6d.h declares (tests check that the library exports exactly these)
 SYMBOLS = (
     "bsl6d_create", "bsl6d_destroy", "bsl6d_advect", "bsl6d_advect_generic", "bsl6d_rotate",
-    "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_strerror", "bsl6d_last_cuda_error",
+    "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_run_host_begin", "bsl6d_run_host_end", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
     "bsl6d_advect_pointwise", "bsl6d_set_boundary",
@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
     lib.bsl6d_strang_step.argtypes = [vp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, vp]
     lib.bsl6d_density.argtypes = [vp, dp, dp, vp]
     lib.bsl6d_run_host.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int]
+    lib.bsl6d_run_host_begin.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int, C.c_int]
+    lib.bsl6d_run_host_end.argtypes = [vp, C.c_int]
     lib.bsl6d_strerror.argtypes = [C.c_int]
     lib.bsl6d_strerror.restype = C.c_char_p
     lib.bsl6d_last_cuda_error.argtypes = [vp]
@@ -288,26 +290,38 @@ class Context:
                     "bsl6d_density")
         return rho
 
-    def run_host(self, f_in_host, f_out_host, ops: Sequence[dict]):
-        """ops: dicts with kind in {'advect','rotate','density'} and dim / shift_source / dt / B / rho_host."""
-        self._shape_ok(f_in_host, "f_in_host"); self._shape_ok(f_out_host, "f_out_host")
+    def _host_ops(self, ops: Sequence[dict]):
         arr = (HostOp * max(1, len(ops)))()
-        keep = []
         for i, op in enumerate(ops):
             kind = {"advect": 0, "rotate": 1, "density": 2}[op["kind"]]
             arr[i].kind = kind
             arr[i].dim = int(op.get("dim", 0))
             arr[i].dt = float(op.get("dt", 0.0))
-            ss = op.get("shift_source")
-            arr[i].shift_source = _host_ptr(ss, "shift_source")
-            rho = op.get("rho_host")
-            arr[i].rho_host = _host_ptr(rho, "rho_host")
+            arr[i].shift_source = _host_ptr(op.get("shift_source"), "shift_source")
+            arr[i].rho_host = _host_ptr(op.get("rho_host"), "rho_host")
             for k, b in enumerate(op.get("B", (0.0, 0.0, 0.0))):
                 arr[i].B[k] = float(b)
-            keep += [ss, rho]
+        return arr
+
+    def run_host(self, f_in_host, f_out_host, ops: Sequence[dict]):
+        """ops: dicts with kind in {'advect','rotate','density'} and dim / shift_source / dt / B / rho_host."""
+        self._shape_ok(f_in_host, "f_in_host"); self._shape_ok(f_out_host, "f_out_host")
+        arr = self._host_ops(ops)
         self._check(self._lib.bsl6d_run_host(self._h, _host_ptr(f_in_host, "f_in_host"),
                                              _host_ptr(f_out_host, "f_out_host"), arr, len(ops)), "bsl6d_run_host")
         return f_out_host
+
+    def run_host_begin(self, f_in_host, f_out_host, ops: Sequence[dict], slot: int):
+        """Enqueue upload, ops and download on `slot` (0 or 1) without waiting; the caller keeps every host tensor of
+        the call alive and untouched until run_host_end(slot)."""
+        self._shape_ok(f_in_host, "f_in_host"); self._shape_ok(f_out_host, "f_out_host")
+        arr = self._host_ops(ops)
+        self._check(self._lib.bsl6d_run_host_begin(self._h, _host_ptr(f_in_host, "f_in_host"),
+                                                   _host_ptr(f_out_host, "f_out_host"), arr, len(ops), int(slot)),
+                    "bsl6d_run_host_begin")
+
+    def run_host_end(self, slot: int):
+        self._check(self._lib.bsl6d_run_host_end(self._h, int(slot)), "bsl6d_run_host_end")
 
     # -- introspection --------------------------------------------------------------------------------------
     def launch_count(self) -> int:

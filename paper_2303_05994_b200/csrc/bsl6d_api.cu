@@ -48,10 +48,10 @@ struct bsl6d_ctx {
     size_t smem_ok_bytes[64];
     int n_smem_ok;
     // host-path working set (bsl6d_run_host), allocated on first use
-    double* h_f;              // device buffer for f
-    double* h_small;          // device buffer for shift sources / rho
-    size_t h_small_cap;
-    cudaStream_t h_stream;
+    double* h_f[2];           // device buffer for f, per slot (bsl6d_run_host_begin keeps two steps in flight)
+    double* h_small[2];       // device buffer for shift sources / rho, per slot
+    size_t h_small_cap[2];
+    cudaStream_t h_stream[2];
 };
 
 namespace {
@@ -988,9 +988,11 @@ int bsl6d_create(const bsl6d_grid* grid, int degree, bsl6d_ctx** out) {
 
 void bsl6d_destroy(bsl6d_ctx* c) {
     if (!c) return;
-    if (c->h_stream) { cudaStreamSynchronize(c->h_stream); cudaStreamDestroy(c->h_stream); }
-    cudaFree(c->h_f);
-    cudaFree(c->h_small);
+    for (int sl = 0; sl < 2; ++sl) {
+        if (c->h_stream[sl]) { cudaStreamSynchronize(c->h_stream[sl]); cudaStreamDestroy(c->h_stream[sl]); }
+        cudaFree(c->h_f[sl]);
+        cudaFree(c->h_small[sl]);
+    }
     for (int k = 0; k < 5; ++k) cudaFree(c->fld[k]);
     for (int k = 0; k < 3; ++k) cudaFree(c->tw[k]);
     cudaFree(c->d_part);
@@ -1244,8 +1246,9 @@ int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     return BSL6D_OK;
 }
 
-int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, const bsl6d_host_op* ops, int nops) {
-    if (!c || !f_in_host || !f_out_host || nops < 0 || (nops > 0 && !ops)) return BSL6D_EINVAL;
+int bsl6d_run_host_begin(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, const bsl6d_host_op* ops, int nops,
+                         int slot) {
+    if (!c || !f_in_host || !f_out_host || nops < 0 || (nops > 0 && !ops) || slot < 0 || slot > 1) return BSL6D_EINVAL;
     if (int rcd = check_device(c)) return rcd;
     const bsl6d_grid& g = c->g;
     const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
@@ -1271,24 +1274,24 @@ int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, co
         }
     }
     cudaError_t e;
-    if (!c->h_stream) {
-        e = cudaStreamCreateWithFlags(&c->h_stream, cudaStreamNonBlocking);
+    if (!c->h_stream[slot]) {
+        e = cudaStreamCreateWithFlags(&c->h_stream[slot], cudaStreamNonBlocking);
         if (e != cudaSuccess) return cuda_fail(c, e);
     }
-    if (!c->h_f) {
-        e = cudaMalloc((void**)&c->h_f, bytes);
-        if (e != cudaSuccess) { (void)cudaGetLastError(); c->h_f = nullptr; return BSL6D_ENOMEM; }
+    if (!c->h_f[slot]) {
+        e = cudaMalloc((void**)&c->h_f[slot], bytes);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); c->h_f[slot] = nullptr; return BSL6D_ENOMEM; }
     }
-    if (small > c->h_small_cap) {
-        cudaFree(c->h_small);
-        c->h_small = nullptr;
-        c->h_small_cap = 0;
-        e = cudaMalloc((void**)&c->h_small, small * sizeof(double));
+    if (small > c->h_small_cap[slot]) {
+        cudaFree(c->h_small[slot]);
+        c->h_small[slot] = nullptr;
+        c->h_small_cap[slot] = 0;
+        e = cudaMalloc((void**)&c->h_small[slot], small * sizeof(double));
         if (e != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
-        c->h_small_cap = small;
+        c->h_small_cap[slot] = small;
     }
-    cudaStream_t st = c->h_stream;
-    e = cudaMemcpyAsync(c->h_f, f_in_host, bytes, cudaMemcpyHostToDevice, st);
+    cudaStream_t st = c->h_stream[slot];
+    e = cudaMemcpyAsync(c->h_f[slot], f_in_host, bytes, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(c, e);
     size_t off = 0;
     int rc = BSL6D_OK;
@@ -1298,30 +1301,44 @@ int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, co
             const double* dsrc = nullptr;
             if (op.shift_source) {
                 const size_t cnt = op.dim < 3 ? (size_t)g.n[op.dim + 3] : nx;
-                e = cudaMemcpyAsync(c->h_small + off, op.shift_source, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
+                e = cudaMemcpyAsync(c->h_small[slot] + off, op.shift_source, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
                 if (e != cudaSuccess) { rc = cuda_fail(c, e); break; }
-                dsrc = c->h_small + off;
+                dsrc = c->h_small[slot] + off;
                 off += cnt;
             }
-            rc = bsl6d_advect(c, c->h_f, c->h_f, op.dim, dsrc, op.dt, st);
+            rc = bsl6d_advect(c, c->h_f[slot], c->h_f[slot], op.dim, dsrc, op.dt, st);
         } else if (op.kind == 1) {
-            rc = bsl6d_rotate(c, c->h_f, c->h_f, op.B, op.dt, st);
+            rc = bsl6d_rotate(c, c->h_f[slot], c->h_f[slot], op.B, op.dt, st);
         } else {
-            rc = bsl6d_density(c, c->h_f, c->h_small + off, st);
+            rc = bsl6d_density(c, c->h_f[slot], c->h_small[slot] + off, st);
             if (rc == BSL6D_OK) {
-                e = cudaMemcpyAsync(op.rho_host, c->h_small + off, nx * sizeof(double), cudaMemcpyDeviceToHost, st);
+                e = cudaMemcpyAsync(op.rho_host, c->h_small[slot] + off, nx * sizeof(double), cudaMemcpyDeviceToHost, st);
                 if (e != cudaSuccess) rc = cuda_fail(c, e);
             }
             off += nx;
         }
     }
     if (rc == BSL6D_OK) {
-        e = cudaMemcpyAsync(f_out_host, c->h_f, bytes, cudaMemcpyDeviceToHost, st);
+        e = cudaMemcpyAsync(f_out_host, c->h_f[slot], bytes, cudaMemcpyDeviceToHost, st);
         if (e != cudaSuccess) rc = cuda_fail(c, e);
     }
-    e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess && rc == BSL6D_OK) rc = cuda_fail(c, e);
+    if (rc != BSL6D_OK) (void)cudaStreamSynchronize(st);    // leave nothing of a failed call in flight
     return rc;
+}
+
+int bsl6d_run_host_end(bsl6d_ctx* c, int slot) {
+    if (!c || slot < 0 || slot > 1) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
+    if (!c->h_stream[slot]) return BSL6D_OK;               // nothing was ever begun on this slot
+    cudaError_t e = cudaStreamSynchronize(c->h_stream[slot]);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return BSL6D_OK;
+}
+
+int bsl6d_run_host(bsl6d_ctx* c, const double* f_in_host, double* f_out_host, const bsl6d_host_op* ops, int nops) {
+    int rc = bsl6d_run_host_begin(c, f_in_host, f_out_host, ops, nops, 0);
+    if (rc != BSL6D_OK) return rc;
+    return bsl6d_run_host_end(c, 0);
 }
 
 }  // extern "C"

@@ -392,6 +392,25 @@ def test_run_host_matches_device_path():
     assert torch.equal(out_h, g.cpu()) and torch.equal(rho_h, rho.cpu())
     ref = oracle.strang_step(ogrid(w), w.degree, f.numpy().copy(), w.E(), w.B, w.dt)
     assert_close(out_h.numpy(), ref, "run_host strang")
+    # two problems in flight (bsl6d_run_host_begin / _end on slots 0 and 1, then a third queued behind slot 0):
+    # the same numbers as one after the other
+    ins = [f.pin_memory(), (f * 0.5 + 0.01).pin_memory(), (f * 2.0).pin_memory()]
+    outs = [torch.empty_like(f).pin_memory() for _ in ins]
+    rhos = [torch.empty(w.n[:3], dtype=torch.float64).pin_memory() for _ in ins]
+    with ctx_for(w) as ctx:
+        for k in range(3):
+            ctx.run_host_begin(ins[k], outs[k], ops[:-1] + [dict(kind="density", rho_host=rhos[k])], k % 2)
+        ctx.run_host_end(0)
+        ctx.run_host_end(1)
+        for k in range(3):
+            o1 = torch.empty_like(f)
+            r1 = torch.empty(w.n[:3], dtype=torch.float64)
+            ctx.run_host(ins[k], o1, ops[:-1] + [dict(kind="density", rho_host=r1)])
+            assert torch.equal(outs[k], o1) and torch.equal(rhos[k], r1), k
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.run_host_begin(ins[0], outs[0], ops, 2)
+        assert e.value.code == bsl.EINVAL
+        ctx.run_host_end(1)                                  # nothing pending: returns at once
 
 
 def test_error_codes():
