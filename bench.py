@@ -595,11 +595,14 @@ def measure_e2e(G: Gpu, w, f0_host, K: int):
            "h2d_bytes_per_step": 8 * w.npts + 8 * n_small, "d2h_bytes_per_step": 8 * w.npts + 8 * nx,
            "steps": ke, "ms_per_step": serial["ms_per_step"], "api": "bsl6d_run_host (pinned host buffers)",
            "workload": workload_label(w)}
-    # ---- two steps in flight: both slots upload f0_host (read only here), each downloads into a buffer of its own ----
+    # ---- two steps in flight: both slots upload f0_host (read only here) and download into ONE more pinned buffer.
+    # A user with two problems gives each its own output; here every step is the same problem, so the two downloads
+    # carry the same bytes and one buffer (29 GB less pinned memory per rank at C5) serves both. ----
     free_dev = torch.cuda.mem_get_info()[0]
-    ok = host_memory_allows(2 * 8 * w.npts * G.world, factor=1.5) and free_dev > 1.2 * 8 * w.npts
+    ok = host_memory_allows(8 * w.npts * G.world, factor=1.5) and free_dev > 1.2 * 8 * w.npts
     if max_over_ranks(0.0 if ok else 1.0, G.dev) == 0.0:
-        outs = [torch.empty(w.n, dtype=torch.float64, pin_memory=True) for _ in range(2)]
+        out = torch.empty(w.n, dtype=torch.float64, pin_memory=True)
+        outs = [out, out]
         hops2 = [hops, make_ops()[0]]
         kp = max(4, 2 * ke)
         for sl in (0, 1):                                     # warm-up: allocates the second slot's device buffer
@@ -621,7 +624,7 @@ def measure_e2e(G: Gpu, w, f0_host, K: int):
                     "api": "bsl6d_run_host_begin / bsl6d_run_host_end, two steps in flight (pinned host buffers): "
                            "the upload of step k+1 overlaps the download of step k",
                     "serial": serial})
-        del outs
+        del outs, out
     ctx.destroy()
     return rec
 
