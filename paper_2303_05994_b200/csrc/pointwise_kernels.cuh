@@ -209,10 +209,9 @@ __global__ void __launch_bounds__(T) pointwise_generic_kernel(const PointwiseArg
 
 // unit-stride dim (inner == 1, always a v dim), extent N compiled in: PB pencils per block, f and alpha transposed
 // through two padded shared-memory tiles (odd row pitch: "lane = pencil" accesses are conflict-free; filled by
-// asynchronous copies, see below); results overwrite
-// the alpha tile (alpha_j is consumed by the one thread that produces out_j).  A pencil is cut into S segments of
-// R = ceil(N/S) outputs, one thread each (the lanes of a warp share the segment): a thread holds R+Q-1 values
-// instead of N, so that a block has S times the warps for the same tile.
+// asynchronous copies, see below); results overwrite the alpha tile (alpha_j is consumed by the one thread that
+// produces out_j).  A pencil is cut into S segments of R = ceil(N/S) outputs, one thread each (the lanes of a warp
+// share the segment): a thread holds R+Q-1 values instead of N, so that a block has S times the warps for the same tile.
 template <int N, int Q, int S, int PB, int MINB>
 __global__ void __launch_bounds__(PB * S, MINB) pointwise_unit_kernel(const PointwiseArgs a) {
     extern __shared__ double tiles[];                      // 2 x PB x LD
