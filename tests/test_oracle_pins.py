@@ -180,6 +180,40 @@ def test_mass_conservation_periodic(q):
 
 
 # ------------------------------------------------------------------------------------------------
+# a whole periodic sweep in closed form: a single Fourier mode is an eigenvector of the sweep
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("q", (4, 6, 8, 10))
+def test_single_fourier_mode_is_multiplied_by_the_symbol(q):
+    """f_j = cos(kappa j + phase) on a periodic pencil: the sweep with displacement alpha = k + theta returns
+    Re(g e^{i(kappa j + phase)}) with the symbol g = sum_m w_m(theta) e^{i kappa (k+m)} (the weights here from the
+    exact-rational solve, not from the oracle).  A wrong stencil offset, a transposed weight vector or a wrong wrap
+    changes the phase of g; |g| -> 1 and arg g -> kappa*alpha as the mode gets smoother (order q)."""
+    n = 32
+    j = np.arange(n)
+    for mode in (1, 3, 7):
+        kappa = 2.0 * math.pi * mode / n
+        for alpha in (0.37, -0.81, 2.25, -5.5, 40.125):
+            k = math.floor(alpha)
+            theta = Fraction(alpha) - k
+            w = np.array([float(v) for v in exact_weights(q, theta)])
+            ms = np.arange(-q // 2 + 1, q // 2 + 1)
+            g = np.sum(w * np.exp(1j * kappa * (k + ms)))
+            for phase in (0.0, 0.6):
+                f = np.cos(kappa * j + phase)[None, :]
+                out = oracle.sweep_pencils(f, np.ones(1), -alpha, q, periodic=True)[0]
+                ref = np.real(g * np.exp(1j * (kappa * j + phase)))
+                assert np.max(np.abs(out - ref)) < 2e-14, (q, mode, alpha)
+        # consistency of the symbol with the exact shift e^{i kappa alpha}: error falls like kappa^q
+    errs = []
+    for mode in (1, 2):
+        kappa = 2.0 * math.pi * mode / n
+        w = np.array([float(v) for v in exact_weights(q, Fraction(1, 2))])
+        ms = np.arange(-q // 2 + 1, q // 2 + 1)
+        errs.append(abs(np.sum(w * np.exp(1j * kappa * ms)) - np.exp(1j * kappa * 0.5)))
+    assert errs[0] < errs[1] and errs[1] / errs[0] > 2.0 ** (q - 0.5)
+
+
+# ------------------------------------------------------------------------------------------------
 # whole-pencil check against scipy's barycentric Lagrange routine and against exact rationals
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("q", (4, 6, 8, 10))
