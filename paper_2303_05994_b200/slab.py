@@ -14,6 +14,13 @@ slabs, with device copies, and sequences C-ABI calls.  Every arithmetic step run
   * interior context: grid (L, n1..n5) on the interior view of the local array -- sweeps along dims 1-5, rotate, density;
   * x1 context: grid (L + 2w, n1..n5) with bsl6d_set_boundary(0, open) -- the x1 sweep over interior + halos.
 The interior results are bit-identical to the same operation on the undivided grid (tests/test_gpu_slab.py).
+
+Overlap (by eq (9) the x1 sweep is communication-bound, so the exchange "must be overlapped with the
+interior"): the planes a neighbour needs -- the lowest and the highest w interior planes -- are brought up to date
+FIRST (every operation between two x1 sweeps acts plane by plane, so it can run on the two boundary regions before the
+middle), the exchange is posted, and the middle planes are computed while the halos travel
+(Slab.strang_step_overlapped; exchange_start / exchange_finish).  Sub-slab contexts (grids of w or L-2w planes) do the
+regional work; results stay bit-identical.  With halos as thick as half a slab (L = 2w) nothing is left to overlap.
 Measured on hardware: single GPU only (this environment has one GPU per run); the N > 1 path is covered by the
 world_size-2 gloo test of the exchange and by the single-GPU emulation with 2 and 4 slabs.
 """
@@ -75,6 +82,14 @@ class SlabPlan:
     def halo_bytes_per_side(self) -> int:
         return 8 * self.w * self.plane
 
+    @property
+    def regions(self):
+        """Plane ranges of the local array for the overlapped step: (boundary low = send_lo, boundary high = send_hi,
+        middle), or None when the two boundary regions overlap (L < 2w) -- then the whole interior is boundary."""
+        if self.L < 2 * self.w:
+            return None
+        return (self.send_lo, self.send_hi, (2 * self.w, self.L))
+
 
 def plan_slab(n_global: Sequence[int], degree: int, world: int, rank: int, max_shift_cells: float) -> SlabPlan:
     """Halo width: the stencil reaches q/2 nodes beyond the foot cell and the foot lies up to ceil(max|alpha|) cells
@@ -110,14 +125,15 @@ def exchange_local(plans: List[SlabPlan], locals_: List[torch.Tensor]) -> None:
         _planes(locals_[r], p.recv_hi).copy_(_planes(locals_[p.right], plans[p.right].send_lo))
 
 
-def exchange(plan: SlabPlan, f_local: torch.Tensor, group=None):
-    """Periodic-ring halo exchange with the two neighbours over torch.distributed (one send and one receive per side,
-    posted together).  Returns after the halos of f_local are filled."""
+def exchange_start(plan: SlabPlan, f_local: torch.Tensor, group=None):
+    """Post the periodic-ring halo exchange with the two neighbours over torch.distributed (one send and one receive
+    per side, posted together) and return a handle for exchange_finish.  The boundary planes being sent must be final;
+    work on other planes may be enqueued before exchange_finish (NCCL runs the transfers on its own stream)."""
     import torch.distributed as dist
     if plan.world == 1:
         _planes(f_local, plan.recv_lo).copy_(_planes(f_local, plan.send_hi))
         _planes(f_local, plan.recv_hi).copy_(_planes(f_local, plan.send_lo))
-        return
+        return []
     ops = [
         dist.P2POp(dist.isend, _planes(f_local, plan.send_hi), plan.right, group, tag=1),
         dist.P2POp(dist.irecv, _planes(f_local, plan.recv_lo), plan.left, group, tag=1),
@@ -126,9 +142,19 @@ def exchange(plan: SlabPlan, f_local: torch.Tensor, group=None):
     ]
     # With two ranks both neighbours are the same peer.  Every rank posts the same order (hi out, lo in, lo out, hi in),
     # so NCCL's in-order matching per peer pairs my first send with the peer's first receive (gloo matches by tag).
-    reqs = dist.batch_isend_irecv(ops)
-    for r in reqs:
+    return dist.batch_isend_irecv(ops)
+
+
+def exchange_finish(handle) -> None:
+    """Wait for the transfers of exchange_start: the halos are filled when this returns (GPU: when the current stream
+    gets past it)."""
+    for r in handle or ():
         r.wait()
+
+
+def exchange(plan: SlabPlan, f_local: torch.Tensor, group=None):
+    """exchange_start + exchange_finish: returns after the halos of f_local are filled."""
+    exchange_finish(exchange_start(plan, f_local, group))
 
 
 class Slab:
@@ -139,6 +165,7 @@ class Slab:
         self.lo, self.dx, self.degree = tuple(lo), tuple(dx), int(degree)
         self._int: Optional[api.Context] = None
         self._x1: Optional[api.Context] = None
+        self._sub = {}                                     # plane range -> context (overlapped step)
 
     # -- contexts ------------------------------------------------------------------------------------------
     @property
@@ -158,11 +185,26 @@ class Slab:
             self._x1.set_boundary(0, True)
         return self._x1
 
+    def ctx_planes(self, r) -> api.Context:
+        """Context for planes [r[0], r[1]) of the local array (any operation that does not sweep x1)."""
+        key = (int(r[0]), int(r[1]))
+        if key == tuple(self.plan.interior):
+            return self.ctx_interior
+        if key not in self._sub:
+            p = self.plan
+            lo = (self.lo[0] + (p.x1_offset - p.w + key[0]) * self.dx[0],) + self.lo[1:]
+            self._sub[key] = api.create((key[1] - key[0],) + tuple(p.n_global[1:]), lo, self.dx, self.degree)
+        return self._sub[key]
+
+    def launch_count(self) -> int:
+        return sum(c.launch_count() for c in [self._int, self._x1] + list(self._sub.values()) if c is not None)
+
     def destroy(self):
-        for c in (self._int, self._x1):
+        for c in [self._int, self._x1] + list(self._sub.values()):
             if c is not None:
                 c.destroy()
         self._int = self._x1 = None
+        self._sub = {}
 
     # -- storage -------------------------------------------------------------------------------------------
     def alloc(self, device="cuda") -> torch.Tensor:
@@ -218,3 +260,55 @@ class Slab:
         exchange_fn(f_local)
         self.advect_x1(f_local, half)
         ci.advect_seq(v, v, [(1, None, 0, half / self.dx[1]), (2, None, 0, half / self.dx[2])])
+
+    # -- the same step with the exchanges overlapped ------------------------------------------------------------
+    def local_ops(self, f_local: torch.Tensor, r, seq_x, E, B, dt_v: float, dt_rot: float):
+        """On planes [r[0], r[1]) only: the x2/x3 sweeps of seq_x, then (if dt_v is not None) the E sweeps with the
+        matching planes of E, then the rotation.  Everything here acts plane by plane."""
+        lo, hi = int(r[0]), int(r[1])
+        if hi <= lo:
+            return
+        v = f_local[lo:hi]
+        c = self.ctx_planes((lo, hi))
+        seq = list(seq_x)
+        if dt_v is not None and E is not None:
+            w = self.plan.w
+            seq += [(3 + d, E[d][lo - w:hi - w], 0x7, dt_v / self.dx[3 + d]) for d in range(3) if E[d] is not None]
+        if seq:
+            c.advect_seq(v, v, seq)
+        if dt_rot is not None and B is not None:
+            c.rotate(v, v, B, dt_rot)
+
+    def step_regions(self):
+        """(regions computed before the exchange is posted, regions computed while it is in flight)."""
+        reg = self.plan.regions
+        if reg is None:
+            return [self.plan.interior], []
+        return [reg[0], reg[1]], [reg[2]]
+
+    def strang_step_overlapped(self, f_local: torch.Tensor, E, B, dt: float, group=None, pending=None):
+        """The Strang step of strang_step with both halo exchanges overlapped: the boundary regions are advanced first,
+        the exchange is posted, the middle planes follow while the halos travel.  `pending`: the handle this method
+        returned for the previous step (its trailing x2,x3 half-step already posted the exchange for this step's first
+        x1 sweep); None = post it now.  Returns the handle for the next step; finish it with exchange_finish (or pass it
+        on) before reading the halos.  Bit-identical to strang_step."""
+        half = 0.5 * dt
+        seq_x = [(1, None, 0, half / self.dx[1]), (2, None, 0, half / self.dx[2])]
+        first, later = self.step_regions()
+        if pending is None:
+            pending = exchange_start(self.plan, f_local, group)
+        exchange_finish(pending)
+        self.advect_x1(f_local, half)
+        for r in first:
+            self.local_ops(f_local, r, seq_x, E, B, dt, dt)
+        h = exchange_start(self.plan, f_local, group)
+        for r in later:
+            self.local_ops(f_local, r, seq_x, E, B, dt, dt)
+        exchange_finish(h)
+        self.advect_x1(f_local, half)
+        for r in first:
+            self.local_ops(f_local, r, seq_x, None, None, None, None)
+        h = exchange_start(self.plan, f_local, group)
+        for r in later:
+            self.local_ops(f_local, r, seq_x, None, None, None, None)
+        return h

@@ -152,3 +152,69 @@ def test_slab_strang_driver_single_rank_ring():
     s.strang_step(t, Ed, w.B, w.dt, lambda x: slab.exchange(s.plan, x))
     assert torch.equal(s.interior(t), ref)
     s.destroy()
+
+
+@pytest.mark.parametrize("world,n0", [(2, 32), (4, 32), (2, 12)])
+def test_overlapped_strang_steps_on_slabs_equal_undivided(world, n0):
+    """The overlapped step (boundary regions first, exchange posted, middle planes while the halos travel) on 2 and 4
+    slabs, phases in the lock step of a real run with the exchange emulated by device copies: bit-identical to the
+    undivided grid.  (4, 32): L = 2w, no middle; (2, 12): L < 2w, the whole interior is boundary."""
+    _need_gpu()
+    w = wl.replace(wl.C5.reduced((n0, 4, 4, 8, 8, 8)), degree=5)
+    f = w.make_f("cuda")
+    Ed = [torch.from_numpy(e).cuda() for e in w.E()]
+    ref = f.clone()
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for _ in range(2):
+            ctx.strang_step(ref, None, Ed, w.B, w.dt)
+    ss, plans = _slabs(w, world, 6.0 * 0.5 * w.dt / w.dx[0])
+    L, hw = plans[0].L, plans[0].w
+    assert (plans[0].regions is None) == (L < 2 * hw)
+    locs = _scatter(ss, f)
+    Eloc = [[e[r * L:(r + 1) * L].contiguous() for e in Ed] for r in range(world)]
+    half = 0.5 * w.dt
+    seq_x = [(1, None, 0, half / w.dx[1]), (2, None, 0, half / w.dx[2])]
+    first, later = ss[0].step_regions()
+    slab.exchange_local(plans, locs)
+    for _ in range(2):
+        for s, t in zip(ss, locs):
+            s.advect_x1(t, half)
+        for r, (s, t) in enumerate(zip(ss, locs)):
+            for reg in first:
+                s.local_ops(t, reg, seq_x, Eloc[r], w.B, w.dt, w.dt)
+        slab.exchange_local(plans, locs)                     # posted here in a real run ...
+        for r, (s, t) in enumerate(zip(ss, locs)):
+            for reg in later:                                # ... while the middle planes are advanced
+                s.local_ops(t, reg, seq_x, Eloc[r], w.B, w.dt, w.dt)
+        for s, t in zip(ss, locs):
+            s.advect_x1(t, half)
+        for s, t in zip(ss, locs):
+            for reg in first:
+                s.local_ops(t, reg, seq_x, None, None, None, None)
+        slab.exchange_local(plans, locs)
+        for s, t in zip(ss, locs):
+            for reg in later:
+                s.local_ops(t, reg, seq_x, None, None, None, None)
+    assert torch.equal(_gather(ss, locs), ref)
+    for s in ss:
+        s.destroy()
+
+
+def test_overlapped_strang_driver_single_rank_ring():
+    """Slab.strang_step_overlapped with world = 1, two steps chained through the pending handle."""
+    _need_gpu()
+    w = wl.replace(wl.C5.reduced((16, 4, 4, 8, 8, 8)), degree=5)
+    f0 = w.make_f("cuda")
+    Ed = [torch.from_numpy(e).cuda() for e in w.E()]
+    ref = f0.clone()
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        for _ in range(2):
+            ctx.strang_step(ref, None, Ed, w.B, w.dt)
+    s = slab.Slab(w.n, w.lo, w.dx, w.degree, 1, 0, 6.0 * 0.5 * w.dt / w.dx[0])
+    assert s.plan.regions is not None
+    t = s.scatter_from_global(f0, s.alloc())
+    h = s.strang_step_overlapped(t, Ed, w.B, w.dt)
+    h = s.strang_step_overlapped(t, Ed, w.B, w.dt, pending=h)
+    slab.exchange_finish(h)
+    assert torch.equal(s.interior(t), ref)
+    s.destroy()

@@ -84,6 +84,19 @@ def _worker(rank, world, port):
         t[plan.w:plan.w + plan.L] += 0.5
         slab.exchange(plan, t)
         assert torch.all(t[0] == 1000.0 * plan.left + (plan.L - plan.w) + 0.5)
+        # the two halves on a thicker slab: post, change planes that are neither sent nor received, finish
+        plan = slab.plan_slab((24, 2, 3, 2, 2, 2), 3, world, rank, 0.7)
+        reg = plan.regions
+        assert reg is not None and reg[2][1] > reg[2][0] and reg[0] == plan.send_lo and reg[1] == plan.send_hi
+        t = _coded(plan, rank)
+        h = slab.exchange_start(plan, t)
+        t[reg[2][0]:reg[2][1]] += 7.0                        # middle planes: work that overlaps the transfers
+        slab.exchange_finish(h)
+        for k in range(plan.w):
+            assert torch.all(t[k] == 1000.0 * plan.left + (plan.L - plan.w + k))
+            assert torch.all(t[plan.w + plan.L + k] == 1000.0 * plan.right + k)
+        assert torch.all(t[reg[2][0]] == 1000.0 * rank + (reg[2][0] - plan.w) + 7.0)
+        assert slab.plan_slab((12, 2, 3, 2, 2, 2), 3, 3, 0, 0.7).regions is None      # L = 4 < 2w = 6
     finally:
         dist.destroy_process_group()
 
