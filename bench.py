@@ -64,6 +64,9 @@ def parse_args():
     p.add_argument("--sharded", action="store_true",
                    help="instead of N replicas: ONE global grid cut into x1 slabs over the N ranks, with the ring halo "
                         "exchange before every x1 sweep (strong scaling; DESIGN.md section 7)")
+    p.add_argument("--peer", action="store_true",
+                   help="with --sharded: slabs WITHOUT halo planes -- the x1 sweep reads the neighbours' planes through "
+                        "peer memory (bsl6d_advect_x1_peer; CUDA IPC between the ranks), no exchange step")
     p.add_argument("--paper-benchmark", action="store_true",
                    help="instead of the contract step: the paper's own section-5 benchmark (37^6, random per-point "
                         "shifts, odd widths 3/5/7/9, every direction) through bsl6d_advect_pointwise")
@@ -751,6 +754,72 @@ def run_sharded(args, w):
         G.dist.destroy_process_group()
 
 
+def run_sharded_peer(args, w):
+    """One global grid in x1 slabs WITHOUT halo planes (slab.PeerSlab): the x1 sweep of a rank reads the planes it needs
+    from its ring neighbours' arrays through peer memory (NVLink between GPUs; mapped with CUDA IPC), so the halo
+    exchange is the sweep's own loads -- one kernel, no copies, no exchange step; one ring barrier per x1 sweep."""
+    G = Gpu()
+    torch = G.torch
+    from paper_2303_05994_b200 import slab
+    K, W = args.steps, args.warmup
+    B, dt = (w.B, w.dt) if any(w.B) else (ROT_B, w.dt)
+    vmax = max(abs(w.lo[3]), abs(w.lo[3] + (w.n[3] - 1) * w.dx[3]))
+    s = slab.PeerSlab(w.n, w.lo, w.dx, w.degree, G.world, G.rank, vmax * 0.5 * dt / w.dx[0])
+    p = s.plan
+    s.alloc(G.dev)
+    sub = replace(w, n=(p.L,) + tuple(w.n[1:]), lo=(w.lo[0] + p.x1_offset * w.dx[0],) + tuple(w.lo[1:]))
+    sub.fill(s.f)
+    if G.world > 1:
+        descs = [None] * G.world
+        G.dist.all_gather_object(descs, slab.share_buffers(s.buf))
+        s.connect(slab.open_peer_buffers(descs[p.left]), slab.open_peer_buffers(descs[p.right]))
+    else:
+        s.connect(s.buf, s.buf)
+    E = [torch.from_numpy(e[p.x1_offset:p.x1_offset + p.L].copy()).to(G.dev) for e in w.E()]
+    rho = torch.empty((p.L,) + tuple(w.n[1:3]), dtype=torch.float64, device=G.dev)
+    sync = slab.ring_sync if G.world > 1 else (lambda: None)
+
+    def one_step():
+        s.strang_step(E, B, dt, sync=sync)
+        s.ctx.density(s.f, rho)
+
+    for _ in range(max(W, 0)):
+        one_step()
+    G.barrier()
+    l0 = s.ctx.launch_count()
+    clocks = ClockSampler(G.local)
+    clocks.start()
+    time.sleep(0.25)
+    G.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(G.stream)
+    for _ in range(K):
+        one_step()
+    e1.record(G.stream)
+    G.barrier()
+    clk = clocks.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), G.dev)
+    launches = s.ctx.launch_count() - l0
+    assert torch.isfinite(rho).all()
+    if G.rank == 0:
+        cfg = config_dict(w, G.world)
+        cfg["parallelism"] = (f"ONE global grid in x1 slabs over {G.world} rank(s), {p.L} planes each, no halo planes: the x1 "
+                              f"sweep reads {p.w} planes per side from the ring neighbours' arrays through peer memory "
+                              f"({p.halo_bytes_per_side / 1e9:.2f} GB per side and sweep); one ring barrier per x1 sweep")
+        line = {"metric": METRIC, "value": 12 * w.npts * K / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": G.world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clk, "gpu_launches": int(launches),
+                "peer_bytes_read_per_step_per_rank": 4 * p.halo_bytes_per_side, "fusion": "planner default",
+                "e2e": None, "roofline": None, "cpu_baseline": None,
+                "note": "sharded peer mode: the whole-job value of ONE grid; measured on hardware with one rank only in "
+                        "this environment (the neighbours are then the rank's own array)"}
+        print(json.dumps(line), flush=True)
+    G.barrier()
+    s.destroy()
+    if G.world > 1:
+        G.dist.destroy_process_group()
+
+
 def run_paper_benchmark(args):
     """one 1-D interpolation per direction on 37^6 points, random alpha/dx in [-1,1] per
     point, odd stencil widths.  Reports, per width and direction, the time and GB/s in the paper's convention
@@ -815,7 +884,7 @@ def main():
         run_reference(args, w)
         return
     if args.sharded:
-        run_sharded(args, w)
+        (run_sharded_peer if args.peer else run_sharded)(args, w)
         return
     names = args.per_config if args.per_config is not None else ("C2,C3" if args.workload is None else "")
     extra = [wl.CONFIGS[n] for n in names.split(",") if n and n != w.name]

@@ -147,6 +147,22 @@ BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
  * bsl6d_field_* and bsl6d_vp_step need a fully periodic x grid and return BSL6D_EUNSUPPORTED on an opened context. */
 BSL6D_API int bsl6d_set_boundary(bsl6d_ctx* ctx, int dim, int open);
 
+/* The x1 sweep of a slab WITHOUT halo planes and without an exchange step: the planes a pencil needs from the
+ * neighbouring slabs are read where they are.  ctx describes the slab (grid (L, n1, .., n5)); f_in is the slab's own
+ * array, f_left / f_right the arrays of the ring neighbours below and above -- same shape, DEVICE pointers this GPU
+ * can dereference: peer memory of another GPU mapped into this process (the loads then travel over NVLink: compute
+ * and "collective" are one kernel), arrays of other slabs on the same device, or f_in itself (a ring of one: plain
+ * periodic sweep).  halo_planes = w >= q/2 + the largest |displacement| in cells, rounded up, and <= L: the
+ * neighbours' nearest w planes are guaranteed to be used; a foot further away may read zeros (the caller's promise,
+ * as for halo planes).  Slab thicknesses 8/16/32/48/64 run a compiled streaming register kernel, any other thickness
+ * a run-time-extent kernel that stages the pencil and 2w neighbour planes in shared memory.  Out of place only (f_out must not overlap any input: the neighbours are reading f_in meanwhile), and
+ * the neighbours' arrays must hold the state of the same step: synchronise the ring before the call and before
+ * anyone overwrites an input (one barrier per x1 sweep; paper_2303_05994_b200/slab.py PeerSlab).
+ * shift_source as for bsl6d_advect with dim = 0.  Results are bit-identical to the periodic sweep on the undivided
+ * grid (PAPER.md:150-152, 323 describe the halo version this replaces; eq (9) its cost). */
+BSL6D_API int bsl6d_advect_x1_peer(bsl6d_ctx* ctx, const double* f_in, const double* f_left, const double* f_right,
+                         double* f_out, int halo_planes, const double* shift_source, double dt, void* stream);
+
 /* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libbsl6d.so")
 #: every symbol include/bsl6d.h declares (tests check that the library exports exactly these)
 SYMBOLS = (
     "bsl6d_create", "bsl6d_destroy", "bsl6d_advect", "bsl6d_advect_generic", "bsl6d_rotate",
-    "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_run_host_begin", "bsl6d_run_host_end", "bsl6d_strerror", "bsl6d_last_cuda_error",
+    "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_run_host_begin", "bsl6d_run_host_end", "bsl6d_advect_x1_peer", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
     "bsl6d_advect_pointwise", "bsl6d_set_boundary",
@@ -72,6 +72,7 @@ def load_library() -> C.CDLL:
     lib.bsl6d_run_host.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int]
     lib.bsl6d_run_host_begin.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int, C.c_int]
     lib.bsl6d_run_host_end.argtypes = [vp, C.c_int]
+    lib.bsl6d_advect_x1_peer.argtypes = [vp, dp, dp, dp, dp, C.c_int, dp, C.c_double, vp]
     lib.bsl6d_strerror.argtypes = [C.c_int]
     lib.bsl6d_strerror.restype = C.c_char_p
     lib.bsl6d_last_cuda_error.argtypes = [vp]
@@ -244,6 +245,19 @@ class Context:
         if rc < 0:
             self._check(rc, "bsl6d_set_fusion")
         return rc
+
+    def advect_x1_peer(self, f_in, f_left, f_right, f_out, halo_planes: int, shift_source, dt: float, stream=None):
+        """x1 sweep of a slab reading its neighbours' planes in place (peer memory or same device); out of place."""
+        self._shape_ok(f_in, "f_in"); self._shape_ok(f_out, "f_out")
+        for t, nm in ((f_left, "f_left"), (f_right, "f_right")):      # may live on a peer GPU: element count only
+            if t.numel() != self.npts:
+                raise ValueError(f"{nm}: {t.numel()} elements, want {self.npts} for grid {self.n}")
+        self._count_ok(shift_source, self.n[3], "shift_source")
+        self._check(self._lib.bsl6d_advect_x1_peer(self._h, _dev_ptr(f_in, "f_in"), _dev_ptr(f_left, "f_left"),
+                                                   _dev_ptr(f_right, "f_right"), _dev_ptr(f_out, "f_out"),
+                                                   int(halo_planes), _dev_ptr(shift_source, "shift_source"), float(dt),
+                                                   _stream(stream)), "bsl6d_advect_x1_peer")
+        return f_out
 
     def set_boundary(self, dim: int, open_: bool) -> int:
         """Open (zero-extend) or close (periodic) x dim `dim`; returns the old setting (slab decomposition)."""

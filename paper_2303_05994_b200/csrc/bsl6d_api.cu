@@ -231,6 +231,41 @@ const void* generic_unit_by_q(int q) {
 }
 const void* generic_unit_fn(int q, int T) { return T == 64 ? generic_unit_by_q<64>(q) : generic_unit_by_q<32>(q); }
 
+template <int T>
+const void* peer_by_q(int q) {
+    switch (q) {
+        case 2: return (const void*)bsl6d::sweep_peer_kernel<2, T>;
+        case 4: return (const void*)bsl6d::sweep_peer_kernel<4, T>;
+        case 6: return (const void*)bsl6d::sweep_peer_kernel<6, T>;
+        case 8: return (const void*)bsl6d::sweep_peer_kernel<8, T>;
+        case 10: return (const void*)bsl6d::sweep_peer_kernel<10, T>;
+        case 12: return (const void*)bsl6d::sweep_peer_kernel<12, T>;
+        default: return nullptr;
+    }
+}
+
+// The compiled-extent kernel for bsl6d_advect_x1_peer: the streaming sweep with rows taken from the neighbours' arrays.
+template <int N>
+const void* peer_stream_by_q(int q) {
+    switch (q) {
+        case 4: return (const void*)bsl6d::sweep_stream_kernel<N, 4, false, 128, 4, 12, true>;
+        case 6: return (const void*)bsl6d::sweep_stream_kernel<N, 6, false, 128, 4, 12, true>;
+        case 8: return (const void*)bsl6d::sweep_stream_kernel<N, 8, false, 128, 4, 12, true>;
+        case 10: return (const void*)bsl6d::sweep_stream_kernel<N, 10, false, 128, 4, 12, true>;
+        default: return nullptr;
+    }
+}
+const void* peer_stream_fn(int n, int q) {
+    switch (n) {
+        case 8: return peer_stream_by_q<8>(q);
+        case 16: return peer_stream_by_q<16>(q);
+        case 32: return peer_stream_by_q<32>(q);
+        case 48: return peer_stream_by_q<48>(q);
+        case 64: return peer_stream_by_q<64>(q);
+        default: return nullptr;
+    }
+}
+
 // Which kernel serves a sweep along `dim`?  (Also used by bsl6d_kernel_name.)
 int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     const int n = c->g.n[dim];
@@ -1039,6 +1074,87 @@ int bsl6d_advect(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
     }
     if (!shift_source) return BSL6D_EINVAL;
     return launch_sweep(c, f_in, f_out, dim, shift_source, 0x7u, scale, (cudaStream_t)stream);
+}
+
+int bsl6d_advect_x1_peer(bsl6d_ctx* c, const double* f_in, const double* f_left, const double* f_right, double* f_out,
+                         int halo_planes, const double* shift_source, double dt, void* stream) {
+    if (!c || !f_in || !f_left || !f_right || !f_out || !std::isfinite(dt)) return BSL6D_EINVAL;
+    const int32_t* n = c->g.n;
+    if (halo_planes < c->q / 2 || halo_planes > n[0]) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
+    // out of place against all three inputs: the neighbours read this slab's input while it is swept
+    if (f_out == f_in || f_out == f_left || f_out == f_right || partial_overlap(c, f_in, f_out) ||
+        partial_overlap(c, f_left, f_out) || partial_overlap(c, f_right, f_out))
+        return BSL6D_EALIAS;
+    size_t inner = 1;
+    for (int d = 1; d < 6; ++d) inner *= (size_t)n[d];
+    if (inner > 0xFFFFFFFFull) return BSL6D_EUNSUPPORTED;
+    const double* ssrc = shift_source ? shift_source : c->d_nodes + c->node_off[3];
+    if (const void* sfn = peer_stream_fn(n[0], c->q)) {
+        // compiled extent: the streaming register kernel, rows beyond the slab loaded from the neighbours' arrays
+        SweepArgs sa;
+        std::memset(&sa, 0, sizeof(sa));
+        sa.in = f_in;
+        sa.left = f_left;
+        sa.right = f_right;
+        sa.out = f_out;
+        sa.src = ssrc;
+        sa.scale = dt / c->g.dx[0];
+        sa.inner = (uint32_t)inner;
+        sa.outer = 1u;
+        sa.n = (uint32_t)n[0];
+        int rcs = build_src_terms(n, 0, 1u << 3, sa.terms);
+        if (rcs) return rcs;
+        const unsigned T = 128;
+        unsigned grid;
+        if (inner % 32 != 0) {
+            sa.ti_log2 = bsl6d::kFlatPencils;
+            sa.nib = (uint32_t)inner;
+            grid = (unsigned)((inner + T - 1) / T);
+        } else {
+            sa.ti_log2 = ceil_pow2_log2(inner < T ? inner : T);
+            const uint32_t TI = 1u << sa.ti_log2, TO = T / TI;
+            sa.nib = (uint32_t)((inner + TI - 1) / TI);
+            grid = sa.nib * ((1u + TO - 1) / TO);
+        }
+        void* sargs[] = {(void*)&sa};
+        cudaError_t es = cudaLaunchKernel(sfn, dim3(grid), dim3(T), sargs, 0, (cudaStream_t)stream);
+        if (es != cudaSuccess) return cuda_fail(c, es);
+        es = cudaGetLastError();
+        if (es != cudaSuccess) return cuda_fail(c, es);
+        c->launches += 1;
+        return BSL6D_OK;
+    }
+    const size_t rows = (size_t)n[0] + 2 * (size_t)halo_planes;
+    int T = 64;
+    if (rows * T * sizeof(double) > 200 * 1024) T = 32;
+    if (rows * T * sizeof(double) > 200 * 1024) return BSL6D_EUNSUPPORTED;
+    const void* fn = T == 64 ? peer_by_q<64>(c->q) : peer_by_q<32>(c->q);
+    if (!fn) return BSL6D_EUNSUPPORTED;
+    bsl6d::PeerArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.in = f_in;
+    a.left = f_left;
+    a.right = f_right;
+    a.out = f_out;
+    a.src = ssrc;
+    a.scale = dt / c->g.dx[0];
+    a.inner = (uint32_t)inner;
+    a.n = (uint32_t)n[0];
+    a.w = (uint32_t)halo_planes;
+    int rc = build_src_terms(n, 0, 1u << 3, a.terms);
+    if (rc) return rc;
+    const size_t smem = rows * T * sizeof(double);
+    rc = allow_smem(c, fn, smem);
+    if (rc) return rc;
+    void* args[] = {(void*)&a};
+    const unsigned grid = (unsigned)((inner + (size_t)T - 1) / (size_t)T);
+    cudaError_t e = cudaLaunchKernel(fn, dim3(grid), dim3((unsigned)T), args, smem, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return BSL6D_OK;
 }
 
 int bsl6d_rotate(bsl6d_ctx* c, const double* f_in, double* f_out, const double B[3], double dt, void* stream) {

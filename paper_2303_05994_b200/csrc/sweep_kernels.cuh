@@ -56,6 +56,8 @@ struct SweepArgs {
     uint32_t ti_log2;      // strided: threads of a block along `inner` = 1 << ti_log2
     uint32_t nib;          // strided: number of inner chunks (= ceil(inner / TI)); flattened mode: number of pencils
     SrcTerms terms;
+    const double* left;    // sweep_stream_kernel<.., PEER = true> only: the ring neighbours' arrays (same shape as `in`)
+    const double* right;
 };
 
 // ---- a2: Lagrange basis on the nodes m_i = i - Q/2 + 1, i = 0..Q-1 ------------------------------------------
@@ -205,8 +207,12 @@ __global__ void __launch_bounds__(T, MINB) sweep_strided_kernel(const SweepArgs 
 // long pencils with wide stencils (N = 48, Q = 10: 162-168 registers, 12 warps per SM in sweep_strided_kernel) this
 // roughly halves the registers.  Periodic pencils keep their first Q-1 rows for the wrap at the end.  Arithmetic and
 // its order are those of sweep_strided_kernel: bit-identical results.
-template <int N, int Q, bool PERIODIC, int T, int MINB, int D>
+// PEER = true (x1 sweep of a slab, outer == 1, see sweep_peer_kernel below): the N planes of the slab continue into the
+// neighbours' arrays -- virtual plane r < 0 is plane r+N of a.left, r >= N is plane r-N of a.right -- so the only
+// change is WHERE a row is loaded from; there is no wrap (PERIODIC must be false) and no zero fill within one slab width.
+template <int N, int Q, bool PERIODIC, int T, int MINB, int D, bool PEER = false>
 __global__ void __launch_bounds__(T, MINB) sweep_stream_kernel(const SweepArgs a) {
+    static_assert(!(PEER && PERIODIC), "a slab's pencil does not wrap: it continues into its neighbours");
     const uint32_t tp = threadIdx.x;
     uint32_t i, o;
     bool live;
@@ -245,6 +251,12 @@ __global__ void __launch_bounds__(T, MINB) sweep_stream_kernel(const SweepArgs a
         if (PERIODIC) {
             if (row >= N) row -= N;
             return BSL6D_LD(pin + (size_t)row * stride);
+        }
+        if (PEER) {                                        // outer == 1: the pencil's offset in every array is i
+            if (row < -N || row >= 2 * N) return 0.0;
+            const double* b = row < 0 ? a.left + (size_t)(row + N) * stride
+                                      : (row >= N ? a.right + (size_t)(row - N) * stride : a.in + (size_t)row * stride);
+            return BSL6D_LD(b + i);
         }
         return (row >= 0 && row < N) ? BSL6D_LD(pin + (size_t)row * stride) : 0.0;
     };
@@ -425,6 +437,70 @@ __global__ void __launch_bounds__(T) sweep_generic_kernel(const SweepArgs a, int
 #pragma unroll
         for (int m = 1; m < Q; ++m) acc = fma(w[m], win[m], acc);
         __stcs(a.out + base + (size_t)j * stride, acc);
+    }
+}
+
+// ---- x1 sweep of a SLAB whose neighbours' planes are read where they are ---------------
+// The slab holds planes 0..n-1 of its part of dim 0; the w planes below come from the END of `left`'s array and the
+// w planes above from the START of `right`'s (both arrays have the slab's own shape: n planes).  left / right may be
+// peer memory of another GPU (loads travel over NVLink: the halo "exchange" IS the sweep's own loads -- no halo
+// planes, no copy, no separate communication step), arrays of other slabs on the same device, or `in` itself (one
+// slab: the periodic ring closes on itself).  Out of place only: the neighbours read this slab's input meanwhile.
+// Structure and arithmetic of sweep_generic_kernel (pencil staged in shared memory by cp.async, sliding register
+// window): results are bit-identical to the periodic sweep on the undivided grid as long as no foot lies more than
+// w - q/2 cells away (the caller's promise, as for halo planes; rows beyond the staged range read as zero).
+struct PeerArgs {
+    const double* in;
+    const double* left;
+    const double* right;
+    double* out;
+    const double* src;
+    double scale;
+    uint32_t inner;        // product of the extents of dims 1..5
+    uint32_t n;            // planes of this slab
+    uint32_t w;            // neighbour planes staged on either side (<= n)
+    uint32_t pad_;
+    SrcTerms terms;
+};
+
+template <int Q, int T>
+__global__ void __launch_bounds__(T) sweep_peer_kernel(const PeerArgs a) {
+    extern __shared__ double tile[];                       // (n + 2w) * T
+    const uint32_t i = blockIdx.x * T + threadIdx.x;
+    if (i >= a.inner) return;
+    const int n = (int)a.n, w = (int)a.w;
+    long long k;
+    double theta;
+    split_shift(__ldg(a.src + src_offset(a.terms, 0u, i)), a.scale, k, theta);
+    const size_t stride = a.inner;
+    double* col = tile + threadIdx.x;
+    {
+        const uint32_t dcol = (uint32_t)__cvta_generic_to_shared(col);
+        for (int r = -w; r < n + w; ++r) {                 // virtual plane r -> whose array, which plane
+            const double* src = r < 0 ? a.left + (size_t)(r + n) * stride
+                                      : (r >= n ? a.right + (size_t)(r - n) * stride : a.in + (size_t)r * stride);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dcol + (uint32_t)((r + w) * T * 8)), "l"(src + i) : "memory");
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+    }
+    double wgt[Q];
+    lagrange_weights<Q>(theta, wgt);
+    const long long lim = 2LL * n + 32;
+    long long kk = k + (long long)(1 - Q / 2);
+    kk = kk < -lim ? -lim : (kk > lim ? lim : kk);
+    int row = (int)kk;                                      // virtual plane of the first stencil node of output 0
+    auto fetch = [&](int r) -> double { return (r >= -w && r < n + w) ? col[(r + w) * T] : 0.0; };
+    double win[Q];
+#pragma unroll
+    for (int m = 0; m < Q - 1; ++m) win[m + 1] = fetch(row++);
+    for (int j = 0; j < n; ++j) {
+#pragma unroll
+        for (int m = 0; m < Q - 1; ++m) win[m] = win[m + 1];
+        win[Q - 1] = fetch(row++);
+        double acc = wgt[0] * win[0];
+#pragma unroll
+        for (int m = 1; m < Q; ++m) acc = fma(wgt[m], win[m], acc);
+        __stcs(a.out + (size_t)j * stride + i, acc);
     }
 }
 

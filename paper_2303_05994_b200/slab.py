@@ -312,3 +312,86 @@ class Slab:
         for r in later:
             self.local_ops(f_local, r, seq_x, None, None, None, None)
         return h
+
+
+# ---- slabs WITHOUT halo planes: the x1 sweep reads the neighbours' planes through peer memory -------------------------
+class PeerSlab:
+    """One rank's slab as two plain arrays of L planes (ping-pong); the x1 sweep (bsl6d_advect_x1_peer) reads the w
+    planes it needs from the neighbours' arrays where they are -- peer memory over NVLink when the neighbours are other
+    GPUs, the same device in the single-process emulation -- so there are no halo planes, no exchange step and no
+    halo traffic beyond the sweep's own loads: compute and communication are one kernel.  Everything else acts on the
+    local array in place.  The ring must be synchronised before each x1 sweep (the neighbours' arrays must hold the
+    state of the same step, and nobody may still be reading the buffer this sweep writes): `sync` does that --
+    device synchronise + process-group barrier in a real run, nothing when one process steps all slabs in turn."""
+
+    def __init__(self, n_global, lo, dx, degree: int, world: int, rank: int, max_shift_cells: float):
+        self.plan = plan_slab(n_global, degree, world, rank, max_shift_cells)
+        p = self.plan
+        self.lo, self.dx, self.degree = tuple(lo), tuple(dx), int(degree)
+        lo_loc = (self.lo[0] + p.x1_offset * self.dx[0],) + self.lo[1:]
+        self.ctx = api.create((p.L,) + tuple(p.n_global[1:]), lo_loc, self.dx, self.degree)
+        self.shape = (p.L,) + tuple(p.n_global[1:])
+        self.buf = None            # [X, Y]
+        self.cur = 0               # which buffer holds the state
+        self.left = None           # [X, Y] of the ring neighbours (tensors this process can dereference)
+        self.right = None
+
+    def alloc(self, device="cuda"):
+        self.buf = [torch.zeros(self.shape, dtype=torch.float64, device=device) for _ in range(2)]
+        return self.buf
+
+    def connect(self, left_bufs, right_bufs):
+        """left_bufs / right_bufs: the neighbours' [X, Y] (same process), or what open_peer_buffers returned."""
+        self.left, self.right = list(left_bufs), list(right_bufs)
+
+    @property
+    def f(self) -> torch.Tensor:
+        return self.buf[self.cur]
+
+    def destroy(self):
+        self.ctx.destroy()
+
+    def advect_x1(self, dt: float):
+        c = self.cur
+        self.ctx.advect_x1_peer(self.buf[c], self.left[c], self.right[c], self.buf[1 - c], self.plan.w, None, dt)
+        self.cur = 1 - c
+
+    def local_part(self, E, B, dt_x: float, dt_v, dt_rot):
+        f = self.f
+        seq = [(1, None, 0, dt_x / self.dx[1]), (2, None, 0, dt_x / self.dx[2])]
+        if dt_v is not None and E is not None:
+            seq += [(3 + d, E[d], 0x7, dt_v / self.dx[3 + d]) for d in range(3) if E[d] is not None]
+        self.ctx.advect_seq(f, f, seq)
+        if dt_rot is not None and B is not None:
+            self.ctx.rotate(f, f, B, dt_rot)
+
+    def strang_step(self, E, B, dt: float, sync=lambda: None):
+        half = 0.5 * dt
+        sync()
+        self.advect_x1(half)
+        self.local_part(E, B, half, dt, dt)
+        sync()
+        self.advect_x1(half)
+        self.local_part(None, None, half, None, None)
+
+
+def ring_sync(group=None):
+    """Barrier for PeerSlab.strang_step in a multi-process run: every rank's device work is complete, then all ranks
+    meet.  (One per x1 sweep; a few tens of microseconds against sweeps of milliseconds.)"""
+    import torch.distributed as dist
+    torch.cuda.synchronize()
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.barrier(group)
+
+
+def share_buffers(bufs):
+    """Picklable CUDA-IPC descriptions of this rank's arrays, to be sent to the neighbours (all_gather_object)."""
+    from torch.multiprocessing.reductions import reduce_tensor
+    return [reduce_tensor(b)[1] for b in bufs]
+
+
+def open_peer_buffers(descs):
+    """Map a neighbour's arrays into this process (cudaIpcOpenMemHandle; peer access over NVLink is enabled by the
+    runtime when the arrays live on another GPU).  The owner must keep them alive."""
+    from torch.multiprocessing.reductions import rebuild_cuda_tensor
+    return [rebuild_cuda_tensor(*d) for d in descs]
