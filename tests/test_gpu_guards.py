@@ -130,3 +130,21 @@ def test_pointwise_sweeps_stay_inside_their_arrays(n, q):
             _check(go.t, ref, (gi, go, ga), f"pointwise n={n} q={q} dim={dim}")
             ctx.advect_pointwise(gi.t, gi.t, dim, ga.t, q)
             _check(gi.t, ref, (gi, ga), f"pointwise in place n={n} q={q} dim={dim}")
+
+
+@pytest.mark.parametrize("n,degree", [((16, 4, 2, 8, 4, 8), 7), ((12, 3, 2, 8, 4, 5), 5)])
+def test_peer_x1_sweep_stays_inside_the_three_arrays(n, degree):
+    """bsl6d_advect_x1_peer (compiled-thickness streaming kernel and run-time-thickness kernel): own array, both
+    neighbours' arrays, the output and the shift source all guarded."""
+    _need()
+    w = mini(n, degree)
+    rng = np.random.default_rng(5)
+    own, left, right = (torch.from_numpy(rng.random(n)).cuda() for _ in range(3))
+    src = torch.from_numpy(rng.uniform(-6.0, 6.0, n[3])).cuda()
+    halo = (degree + 1) // 2 + 2
+    dt = 1.9 * w.dx[0] / 6.0
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        ref = ctx.advect_x1_peer(own, left, right, torch.empty_like(own), halo, src, dt)
+        gs = [Guarded(t) for t in (own, left, right, torch.zeros_like(own), src)]
+        ctx.advect_x1_peer(gs[0].t, gs[1].t, gs[2].t, gs[3].t, halo, gs[4].t, dt)
+        _check(gs[3].t, ref, gs, f"peer x1 sweep n={n}")
