@@ -278,3 +278,30 @@ def test_random_chains_every_planner_mode_equals_single_sweeps(n, degree, seed):
                 for d, s, m, sc in chain_host:
                     ref = oracle.sweep(ref, d, np.ascontiguousarray(s), m, sc, w.degree + 1)
                 assert rel_err(single, ref) <= TOL
+
+
+@pytest.mark.parametrize("n,degree", [((4, 8, 8, 32, 32, 8), 7), ((2, 16, 16, 16, 16, 16), 5), ((2, 8, 32, 32, 8, 8), 9)])
+def test_tile_passes_with_displacements_of_many_cells(n, degree):
+    """Chains over two dims with |alpha| up to 11 cells, both signs, varying per pencil: the persistent tile pass takes
+    its streaming form for some pencils (first stencil row above -q) and the all-loads-first form for the others in the
+    same warp; zero-extended and periodic dims.  Bit-identical to the sweeps one by one, in and out of place."""
+    _need_gpu()
+    w = wl.replace(wl.C2.reduced(n), degree=degree)
+    rng = np.random.default_rng(sum(n) + degree)
+    fd = w.make_f("cuda")
+    for a, b in ((3, 4), (2, 3), (1, 2)):
+        chain = []
+        for d in (a, b, a, b):
+            mask = sum(1 << k for k in range(6) if k not in (d,) and k in (a, b, 0, 5))
+            shape = [w.n[k] for k in range(6) if mask >> k & 1]
+            src = torch.from_numpy(11.0 * (2.0 * rng.random(shape) - 1.0)).cuda()
+            chain.append((d, src, mask, 1.0))
+        with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+            ctx.set_fusion(0)
+            single = ctx.advect_seq(fd, torch.empty_like(fd), chain)
+            for mode in (1, 2, 5):
+                ctx.set_fusion(mode)
+                assert torch.equal(ctx.advect_seq(fd, torch.empty_like(fd), chain), single), (a, b, mode)
+                inp = fd.clone()
+                ctx.advect_seq(inp, inp, chain)
+                assert torch.equal(inp, single), (a, b, mode, "in place")
