@@ -215,21 +215,34 @@ const void* generic_by_q(int q) {
 }
 const void* generic_fn(int q, int T) { return T == 64 ? generic_by_q<64>(q) : generic_by_q<32>(q); }
 
-constexpr int kGenericUnitSegments = 4;                      // threads per pencil in the unit-stride fallback
-template <int T>
+// unit-stride fallback: PB pencils per block, S = ceil(n / RMAX) threads per pencil, RMAX outputs per thread at most
+template <int PB, int RMAX>
 const void* generic_unit_by_q(int q) {
-    constexpr int S = kGenericUnitSegments;
     switch (q) {
-        case 2: return (const void*)bsl6d::sweep_generic_unit_kernel<2, T, S>;
-        case 4: return (const void*)bsl6d::sweep_generic_unit_kernel<4, T, S>;
-        case 6: return (const void*)bsl6d::sweep_generic_unit_kernel<6, T, S>;
-        case 8: return (const void*)bsl6d::sweep_generic_unit_kernel<8, T, S>;
-        case 10: return (const void*)bsl6d::sweep_generic_unit_kernel<10, T, S>;
-        case 12: return (const void*)bsl6d::sweep_generic_unit_kernel<12, T, S>;
+        case 2: return (const void*)bsl6d::sweep_generic_unit_kernel<2, PB, RMAX>;
+        case 4: return (const void*)bsl6d::sweep_generic_unit_kernel<4, PB, RMAX>;
+        case 6: return (const void*)bsl6d::sweep_generic_unit_kernel<6, PB, RMAX>;
+        case 8: return (const void*)bsl6d::sweep_generic_unit_kernel<8, PB, RMAX>;
+        case 10: return (const void*)bsl6d::sweep_generic_unit_kernel<10, PB, RMAX>;
+        case 12: return (const void*)bsl6d::sweep_generic_unit_kernel<12, PB, RMAX>;
         default: return nullptr;
     }
 }
-const void* generic_unit_fn(int q, int T) { return T == 64 ? generic_unit_by_q<64>(q) : generic_unit_by_q<32>(q); }
+// shape of the unit-stride fallback for extent n: pencils per block, segments per pencil, outputs per thread (0: none)
+struct GenericUnitShape { int pb, s, rmax; };
+GenericUnitShape generic_unit_shape(int n) {
+    const int rmax = n <= 256 ? 16 : 32;
+    const int s = (n + rmax - 1) / rmax;
+    if (s > 16) return GenericUnitShape{0, 0, 0};            // extent above 512
+    const int pb = 64 * s <= 512 ? 64 : 32;
+    return GenericUnitShape{pb, s, rmax};
+}
+const void* generic_unit_fn(int q, int n) {
+    const GenericUnitShape g = generic_unit_shape(n);
+    if (!g.pb) return nullptr;
+    if (g.rmax == 16) return g.pb == 64 ? generic_unit_by_q<64, 16>(q) : generic_unit_by_q<32, 16>(q);
+    return generic_unit_by_q<32, 32>(q);
+}
 
 template <int T>
 const void* peer_by_q(int q) {
@@ -276,15 +289,21 @@ int choose_kernel(const bsl6d_ctx* c, int dim, KernelChoice& k) {
     if (inner == 1) ok = !periodic && unit_lookup(n, c->q, k);
     else ok = periodic ? strided_lookup<true>(n, c->q, k) : strided_lookup<false>(n, c->q, k);
     if (ok) return BSL6D_OK;
-    // fallback: pencils staged in shared memory: n * T doubles (strided), 2 * (n|1) * T doubles (unit stride)
+    // fallback: pencils staged in shared memory: n * T doubles (strided), (n|1) * PB doubles (unit stride)
     const size_t cap = 200 * 1024;
-    const size_t per_thread = ((inner == 1 && !periodic) ? 2 * (size_t)(n | 1) : (size_t)n) * sizeof(double);
+    if (inner == 1 && !periodic) {
+        const GenericUnitShape g = generic_unit_shape(n);
+        if (!g.pb) return BSL6D_EUNSUPPORTED;
+        const size_t smem = (size_t)(n | 1) * (size_t)g.pb * sizeof(double);
+        if (smem > cap) return BSL6D_EUNSUPPORTED;
+        k = KernelChoice{nullptr, g.pb * g.s, smem, 2, g.pb, nullptr, 0};      // gen_T = pencils per block
+        return BSL6D_OK;
+    }
+    const size_t per_thread = (size_t)n * sizeof(double);
     int T = 64;
     if (per_thread * T > cap) T = 32;
     if (per_thread * T > cap) return BSL6D_EUNSUPPORTED;
-    // gen_T = pencils per block; the unit-stride fallback runs kGenericUnitSegments threads per pencil
-    const bool unit = inner == 1 && !periodic;
-    k = KernelChoice{nullptr, unit ? T * kGenericUnitSegments : T, per_thread * T, 2, T, nullptr, 0};
+    k = KernelChoice{nullptr, T, per_thread * T, 2, T, nullptr, 0};
     return BSL6D_OK;
 }
 
@@ -422,7 +441,7 @@ int launch_sweep(bsl6d_ctx* c, const double* f_in, double* f_out, int dim, const
 
     cudaError_t e;
     if (kc.kind == 2) {
-        const void* gfn = (inner == 1 && dim >= 3) ? generic_unit_fn(c->q, kc.gen_T) : generic_fn(c->q, kc.gen_T);
+        const void* gfn = (inner == 1 && !is_periodic(c, dim)) ? generic_unit_fn(c->q, n[dim]) : generic_fn(c->q, kc.gen_T);
         if (!gfn) return BSL6D_EUNSUPPORTED;
         rc = allow_smem(c, gfn, kc.smem);
         if (rc) return rc;

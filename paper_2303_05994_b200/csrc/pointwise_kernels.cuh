@@ -282,11 +282,20 @@ __global__ void pointwise_generic_unit_kernel(const PointwiseArgs a) {
     const double* pin = a.in + p0 * n;
     const double* pal = a.alpha + p0 * n;
     double* pout = a.out + p0 * n;
-    for (uint32_t e = threadIdx.x; e < nelem; e += T) {                  // asynchronous fill, as above
-        const uint32_t s = (e / n) * LD + (e % n);
-        const uint32_t df = (uint32_t)__cvta_generic_to_shared(tf + s), da = (uint32_t)__cvta_generic_to_shared(ta + s);
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(df), "l"(pin + e) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(da), "l"(pal + e) : "memory");
+    // (row, col) = (e / n, e % n) advanced by (T / n, T % n) per step instead of two run-time divisions per element
+    const uint32_t un = (uint32_t)n, dq = T / un, dr = T % un;
+    const uint32_t row0 = threadIdx.x / un, col0 = threadIdx.x % un;
+    {
+        uint32_t row = row0, col = col0;
+        for (uint32_t e = threadIdx.x; e < nelem; e += T) {              // asynchronous fill, as above
+            const uint32_t s = row * LD + col;
+            const uint32_t df = (uint32_t)__cvta_generic_to_shared(tf + s), da = (uint32_t)__cvta_generic_to_shared(ta + s);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(df), "l"(pin + e) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(da), "l"(pal + e) : "memory");
+            row += dq;
+            col += dr;
+            if (col >= un) { col -= un; ++row; }
+        }
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
@@ -309,7 +318,15 @@ __global__ void pointwise_generic_unit_kernel(const PointwiseArgs a) {
         }
     }
     __syncthreads();
-    for (uint32_t e = threadIdx.x; e < nelem; e += T) __stcs(pout + e, ta[(e / n) * LD + (e % n)]);
+    {
+        uint32_t row = row0, col = col0;
+        for (uint32_t e = threadIdx.x; e < nelem; e += T) {
+            __stcs(pout + e, ta[row * LD + col]);
+            row += dq;
+            col += dr;
+            if (col >= un) { col -= un; ++row; }
+        }
+    }
 }
 
 }  // namespace bsl6d

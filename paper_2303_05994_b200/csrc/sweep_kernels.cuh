@@ -509,60 +509,90 @@ __global__ void __launch_bounds__(T) sweep_peer_kernel(const PeerArgs a) {
 // odd row pitch, so that "lane = pencil" accesses are conflict-free.  A pencil is cut into S segments of
 // ceil(n/S) outputs, one thread each (the lanes of a warp share the segment), which gives a block S times the warps
 // for the same tile (with one thread per pencil the kernel ran 10 warps per SM: 3.4 TB/s at 36^6).
-template <int Q, int PB, int S>
-__global__ void __launch_bounds__(PB * S) sweep_generic_unit_kernel(const SweepArgs a) {
-    extern __shared__ double tile[];                       // 2 * PB * LD
-    constexpr int T = PB * S;
+// Round 2 (second half): ONE tile instead of two.  The number of segments per pencil is chosen at launch so that a
+// thread forms at most RMAX = 16 (n <= 256; else 32) outputs (S = ceil(n / RMAX) = blockDim.x / PB); it keeps them in registers (fully
+// unrolled, predicated), and after a barrier -- every segment of a row has read its inputs -- writes them over the
+// row.  Half the shared memory per block (twice the resident blocks) and no second tile to fill.
+template <int Q, int PB, int RMAX>
+__global__ void __launch_bounds__(512) sweep_generic_unit_kernel(const SweepArgs a) {
+    extern __shared__ double tile[];                       // PB * LD
+    const uint32_t T = blockDim.x;                         // PB * S
+    const int S = (int)(T / PB);
     const int n = (int)a.n;
     const int LD = n | 1;
-    double* tin = tile;
-    double* tout = tile + (size_t)PB * LD;
     const size_t p0 = (size_t)blockIdx.x * PB;
     const uint32_t np = (uint32_t)(((size_t)a.outer - p0) < (size_t)PB ? ((size_t)a.outer - p0) : (size_t)PB);
     const uint32_t nelem = np * (uint32_t)n;
     const double* pin = a.in + p0 * n;
     double* pout = a.out + p0 * n;
-    for (uint32_t e = threadIdx.x; e < nelem; e += T) {
-        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tin + (e / n) * LD + (e % n));
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(pin + e) : "memory");
+    // element e of the chunk sits at (row, col) = (e / n, e % n): with a run-time n these two divisions per element and
+    // loop (fill, store) were the kernel's largest cost (~80 of its instructions per point), so (row, col) is advanced
+    // by (T / n, T % n) instead -- two divisions per thread
+    const uint32_t un = (uint32_t)n, dq = T / un, dr = T % un;
+    const uint32_t row0 = threadIdx.x / un, col0 = threadIdx.x % un;
+    {
+        uint32_t row = row0, col = col0;
+        for (uint32_t e = threadIdx.x; e < nelem; e += T) {
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + row * LD + col);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(pin + e) : "memory");
+            row += dq;
+            col += dr;
+            if (col >= un) { col -= un; ++row; }
+        }
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
     const uint32_t pl = threadIdx.x % PB;
     const int seg = (int)(threadIdx.x / PB);
-    if (pl < np) {
+    const int R = (n + S - 1) / S;                         // <= RMAX by the choice of S
+    const int j0 = seg * R, j1 = (j0 + R < n) ? j0 + R : n;
+    double res[RMAX];
+    if (pl < np && j0 < n) {
         long long k;
         double theta;
         split_shift(__ldg(a.src + src_offset(a.terms, (uint32_t)(p0 + pl), 0u)), a.scale, k, theta);
         double w[Q];
         lagrange_weights<Q>(theta, w);
-        const int R = (n + S - 1) / S;
-        const int j0 = seg * R, j1 = (j0 + R < n) ? j0 + R : n;
         const long long lim = 2LL * n + 32;
         long long kk = k + (long long)(1 - Q / 2);
         kk = kk < -lim ? -lim : (kk > lim ? lim : kk);
         int row = (int)kk + j0;                            // first stencil node of output j0
-        const double* rin = tin + pl * LD;
-        double* rout = tout + pl * LD;
-        double win[Q];
+        const double* rin = tile + pl * LD;
+        double win[Q];                                     // ring with static indices: win[(r + m) % Q] = node m of output j0 + r
 #pragma unroll
         for (int m = 0; m < Q - 1; ++m) {
-            win[m + 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
+            win[m] = (row >= 0 && row < n) ? rin[row] : 0.0;
             ++row;
         }
-        for (int j = j0; j < j1; ++j) {
 #pragma unroll
-            for (int m = 0; m < Q - 1; ++m) win[m] = win[m + 1];
-            win[Q - 1] = (row >= 0 && row < n) ? rin[row] : 0.0;
-            ++row;
-            double acc = w[0] * win[0];
+        for (int r = 0; r < RMAX; ++r) {
+            if (j0 + r < j1) {
+                win[(r + Q - 1) % Q] = (row >= 0 && row < n) ? rin[row] : 0.0;
+                ++row;
+                double acc = w[0] * win[r % Q];
 #pragma unroll
-            for (int m = 1; m < Q; ++m) acc = fma(w[m], win[m], acc);
-            rout[j] = acc;
+                for (int m = 1; m < Q; ++m) acc = fma(w[m], win[(r + m) % Q], acc);
+                res[r] = acc;
+            }
         }
     }
+    __syncthreads();                                       // every segment of every row has read its inputs
+    if (pl < np && j0 < n) {
+        double* rout = tile + pl * LD + j0;
+#pragma unroll
+        for (int r = 0; r < RMAX; ++r)
+            if (j0 + r < j1) rout[r] = res[r];
+    }
     __syncthreads();
-    for (uint32_t e = threadIdx.x; e < nelem; e += T) __stcs(pout + e, tout[(e / n) * LD + (e % n)]);
+    {
+        uint32_t row = row0, col = col0;
+        for (uint32_t e = threadIdx.x; e < nelem; e += T) {
+            __stcs(pout + e, tile[row * LD + col]);
+            row += dq;
+            col += dr;
+            if (col >= un) { col -= un; ++row; }
+        }
+    }
 }
 
 }  // namespace bsl6d
