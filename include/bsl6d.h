@@ -22,6 +22,8 @@
  *   a negative BSL6D_E* code; a failed call has enqueued nothing.  No exceptions, no printing, no aborts.
  *   There is no CPU fallback anywhere: without a CUDA device bsl6d_create fails with BSL6D_ECUDA.
  *   Preconditions not checked: f finite; |displacement| < 2^30 cells.
+ *   A context is not thread-safe: one host thread at a time per context (several contexts, and several streams with
+ *   one context, are fine).
  */
 #ifndef BSL6D_H
 #define BSL6D_H
