@@ -22,9 +22,10 @@
  *   a negative BSL6D_E* code; a failed call has enqueued nothing.  No exceptions, no printing, no aborts.
  *   There is no CPU fallback anywhere: without a CUDA device bsl6d_create fails with BSL6D_ECUDA.
  *   Preconditions not checked: f finite; |displacement| < 2^30 cells.
- *   A context is not thread-safe: one host thread at a time per context.  Sweeps, rotations and density moments of one
- *   context may be in flight on several streams; bsl6d_field_* / bsl6d_vp_step use work arrays of the context and must
- *   not overlap each other in time, and each bsl6d_run_host slot is one queue.
+ *   A context is not thread-safe: one host thread at a time per context.  Sweeps and rotations of one context may be in
+ *   flight on several streams; bsl6d_density with v-blocks above 32768 points, bsl6d_field_* and bsl6d_vp_step use work
+ *   arrays of the context and must not overlap each other in time; each bsl6d_run_host slot is one queue with work
+ *   arrays of its own.
  */
 #ifndef BSL6D_H
 #define BSL6D_H

@@ -52,6 +52,7 @@ struct bsl6d_ctx {
     double* h_small[2];       // device buffer for shift sources / rho, per slot
     size_t h_small_cap[2];
     cudaStream_t h_stream[2];
+    double* h_part[2];        // density partial sums per slot (split v-blocks only)
 };
 
 namespace {
@@ -1046,6 +1047,7 @@ void bsl6d_destroy(bsl6d_ctx* c) {
         if (c->h_stream[sl]) { cudaStreamSynchronize(c->h_stream[sl]); cudaStreamDestroy(c->h_stream[sl]); }
         cudaFree(c->h_f[sl]);
         cudaFree(c->h_small[sl]);
+        cudaFree(c->h_part[sl]);
     }
     for (int k = 0; k < 5; ++k) cudaFree(c->fld[k]);
     for (int k = 0; k < 3; ++k) cudaFree(c->tw[k]);
@@ -1354,9 +1356,16 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
     return run_sequence_pingpong(c, f, f_tmp, vs, nv, st);
 }
 
+static int density_impl(bsl6d_ctx* c, const double* f, double* rho, double* part, void* stream);
+
 int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     if (!c || !f || !rho) return BSL6D_EINVAL;
     if (int rcd = check_device(c)) return rcd;
+    return density_impl(c, f, rho, c->d_part, stream);
+}
+
+// part: nx * G doubles of scratch for the partial sums of split v-blocks (unused when G == 1)
+static int density_impl(bsl6d_ctx* c, const double* f, double* rho, double* part, void* stream) {
     const bsl6d_grid& g = c->g;
     const size_t seg = (size_t)g.n[3] * g.n[4] * g.n[5];
     const size_t nx = (size_t)g.n[0] * g.n[1] * g.n[2];
@@ -1364,7 +1373,7 @@ int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     const uint32_t G = c->dens_G;
     if (nx * G > 0x7FFFFFFFull) return BSL6D_EUNSUPPORTED;
     const bool vec = (seg % 2 == 0) && (((uintptr_t)f & 15u) == 0);
-    double* out = G == 1 ? rho : c->d_part;
+    double* out = G == 1 ? rho : part;
     constexpr int T = 256;
     cudaStream_t st = (cudaStream_t)stream;
     if (vec) bsl6d::density_kernel<T, true><<<(unsigned)(nx * G), T, 0, st>>>(f, out, seg, G, c->dens_chunk, dv3);
@@ -1373,7 +1382,7 @@ int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->launches += 1;
     if (G > 1) {
-        bsl6d::density_finish_kernel<<<(unsigned)((nx + 255) / 256), 256, 0, st>>>(c->d_part, rho, nx, G, dv3);
+        bsl6d::density_finish_kernel<<<(unsigned)((nx + 255) / 256), 256, 0, st>>>(part, rho, nx, G, dv3);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(c, e);
         c->launches += 1;
@@ -1425,6 +1434,10 @@ int bsl6d_run_host_begin(bsl6d_ctx* c, const double* f_in_host, double* f_out_ho
         if (e != cudaSuccess) { (void)cudaGetLastError(); return BSL6D_ENOMEM; }
         c->h_small_cap[slot] = small;
     }
+    if (c->dens_G > 1 && !c->h_part[slot]) {                // each slot reduces through scratch of its own
+        e = cudaMalloc((void**)&c->h_part[slot], nx * c->dens_G * sizeof(double));
+        if (e != cudaSuccess) { (void)cudaGetLastError(); c->h_part[slot] = nullptr; return BSL6D_ENOMEM; }
+    }
     cudaStream_t st = c->h_stream[slot];
     e = cudaMemcpyAsync(c->h_f[slot], f_in_host, bytes, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(c, e);
@@ -1445,7 +1458,7 @@ int bsl6d_run_host_begin(bsl6d_ctx* c, const double* f_in_host, double* f_out_ho
         } else if (op.kind == 1) {
             rc = bsl6d_rotate(c, c->h_f[slot], c->h_f[slot], op.B, op.dt, st);
         } else {
-            rc = bsl6d_density(c, c->h_f[slot], c->h_small[slot] + off, st);
+            rc = density_impl(c, c->h_f[slot], c->h_small[slot] + off, c->h_part[slot], st);
             if (rc == BSL6D_OK) {
                 e = cudaMemcpyAsync(op.rho_host, c->h_small[slot] + off, nx * sizeof(double), cudaMemcpyDeviceToHost, st);
                 if (e != cudaSuccess) rc = cuda_fail(c, e);

@@ -413,6 +413,30 @@ def test_run_host_matches_device_path():
         ctx.run_host_end(1)                                  # nothing pending: returns at once
 
 
+def test_run_host_two_slots_with_split_v_blocks():
+    """v-blocks above 32768 points are reduced through scratch partial sums: each host-path slot has scratch of its
+    own, so two density moments in flight at once do not disturb each other."""
+    _need_gpu()
+    w = mini((2, 2, 3, 64, 32, 32), 5, seed=11)
+    rng = np.random.default_rng(3)
+    ins = [torch.from_numpy(rng.random(w.n)).pin_memory() for _ in range(4)]
+    outs = [torch.empty(w.n, dtype=torch.float64).pin_memory() for _ in ins]
+    rhos = [torch.empty(w.n[:3], dtype=torch.float64).pin_memory() for _ in ins]
+    with ctx_for(w) as ctx:
+        for k in range(4):
+            ops = [dict(kind="advect", dim=5, dt=0.3, shift_source=torch.ones(w.n[:3], dtype=torch.float64)),
+                   dict(kind="density", rho_host=rhos[k])]
+            ctx.run_host_begin(ins[k], outs[k], ops, k % 2)
+        ctx.run_host_end(0)
+        ctx.run_host_end(1)
+        for k in range(4):
+            g = ins[k].cuda()
+            ctx.advect(g, g, 5, torch.ones(w.n[:3], dtype=torch.float64, device="cuda"), 0.3)
+            rho = torch.empty(w.n[:3], dtype=torch.float64, device="cuda")
+            ctx.density(g, rho)
+            assert torch.equal(outs[k], g.cpu()) and torch.equal(rhos[k], rho.cpu()), k
+
+
 def test_error_codes():
     _need_gpu()
     with pytest.raises(bsl.Bsl6dError) as e:
