@@ -394,4 +394,13 @@ def open_peer_buffers(descs):
     """Map a neighbour's arrays into this process (cudaIpcOpenMemHandle; peer access over NVLink is enabled by the
     runtime when the arrays live on another GPU).  The owner must keep them alive."""
     from torch.multiprocessing.reductions import rebuild_cuda_tensor
-    return [rebuild_cuda_tensor(*d) for d in descs]
+    bufs = [rebuild_cuda_tensor(*d) for d in descs]
+    cur = torch.cuda.current_device()
+    for b in bufs:
+        if b.device.index != cur:
+            # a kernel on THIS device will dereference the neighbour's pointers: make torch switch peer access on
+            # (it does so on the first cross-device copy).  Not exercised on this one-GPU environment.
+            if not torch.cuda.can_device_access_peer(cur, b.device.index):
+                raise RuntimeError(f"cuda:{cur} cannot access cuda:{b.device.index} as a peer")
+            torch.empty(1, dtype=b.dtype, device=f"cuda:{cur}").copy_(b.view(-1)[:1])
+    return bufs
