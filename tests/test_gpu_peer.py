@@ -58,7 +58,16 @@ def test_x1_peer_sweep_equals_undivided(world, dt_cells):
     ss = _ring(w, world, max_shift, f)
     for s in ss:                                                # every slab reads the others' UNCHANGED input buffers
         s.advect_x1(dt)
-    assert torch.equal(_gather(ss), ref)
+    got = _gather(ss)
+    assert torch.equal(got, ref)
+    # and against the oracle directly (the undivided GPU sweep is compared with it in test_gpu_parity.py as well)
+    import oracle
+    og = oracle.Grid(tuple(w.n), tuple(w.lo), tuple(w.dx))
+    oref = oracle.advect(og, w.degree, f.cpu().numpy(), 0, None, dt)
+    if dt_cells == "whole":
+        assert np.array_equal(got.cpu().numpy(), oref)
+    else:
+        assert np.max(np.abs(got.cpu().numpy() - oref)) <= 1e-12 * np.max(np.abs(oref))
     for s in ss:
         s.destroy()
 
