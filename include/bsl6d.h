@@ -58,7 +58,8 @@ enum {
     BSL6D_EALIAS = -2,        /* f_in and f_out overlap partially (exact aliasing f_in == f_out is legal) */
     BSL6D_EUNSUPPORTED = -3,  /* oblique B turning more than 2 pi; extent without a kernel / too large for on-chip staging */
     BSL6D_ECUDA = -4,         /* CUDA runtime failure; see bsl6d_last_cuda_error */
-    BSL6D_ENOMEM = -5         /* host or device allocation failed */
+    BSL6D_ENOMEM = -5,        /* host or device allocation failed */
+    BSL6D_ESCRATCH = -6       /* bsl6d_density_static: the problem needs more than BSL6D_STATIC_SCRATCH_DOUBLES of scratch */
 };
 
 /* Create a context for `grid` and Lagrange degree `degree` (odd, 1..11; stencil width q = degree+1).
@@ -170,6 +171,34 @@ BSL6D_API int bsl6d_advect_x1_peer(bsl6d_ctx* ctx, const double* f_in, const dou
 /* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);
+
+/* ---- the density moment without any allocation ----------------------------------------------------------------
+ * For callers that may not call cudaMalloc / cudaFree (or anything that does): code living inside a host application
+ * that owns all device memory through a pool or caching allocator of its own, diagnostics that run between time steps
+ * and cannot afford the device-wide synchronisation an allocation or a free may bring, jobs so close to the memory
+ * limit that an allocation in mid-run may fail.  Every other entry point needs a context, and bsl6d_create allocates;
+ * this one needs none: it computes the same moment as bsl6d_density (same chunking, same order of additions, the same
+ * bits) from plain arguments, and the scratch that split v-blocks need -- the partial sums, nx*G doubles with
+ * nx = n0*n1*n2 and G = the number of chunks of <= 32768 doubles one v-block n3*n4*n5 is cut into -- sits in a
+ * __device__ array compiled into the library: BSL6D_STATIC_SCRATCH_DOUBLES doubles = 2 MiB, held by every GPU the
+ * library's code is loaded on, from load until the process exits.
+ *   n      HOST, the six extents (each >= 1);   dv: HOST, the spacings of v1, v2, v3 (finite, > 0)
+ *   f      DEVICE, n0*..*n5 doubles, C order, 8-byte aligned (16 for full speed);   rho: DEVICE, n0*n1*n2 doubles
+ *   stream cudaStream_t as void*; the launches (one, or two when G > 1) are enqueued there, no synchronisation
+ *   cuda_error  HOST, may be NULL: receives the cudaError_t when the call returns BSL6D_ECUDA, else 0
+ * f and rho must live on the CURRENT device.  Returns BSL6D_ESCRATCH -- and launches nothing -- when G > 1 and
+ * nx*G > BSL6D_STATIC_SCRATCH_DOUBLES (BASELINE config C3, 16^3 x 64^3, needs 32768; blocks of <= 32768 velocity
+ * points need no scratch at any nx); BSL6D_EUNSUPPORTED when nx*G >= 2^31 or the device ordinal is >= 64.
+ * It calls no cudaMalloc, cudaFree or allocating library routine.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, which may make the runtime load
+ * the library's code onto that device); make that first call outside any stream capture.
+ * Sharing: all calls on a device use the one array and find the previous call's partial sums in it.  Nothing needs
+ * clearing -- a call overwrites each slot it later reads -- but two calls whose kernels may run at the same time
+ * (different streams with no ordering between them, from one host thread or several) race on it and return garbage.
+ * Calls on one stream, or ordered by events, are safe; the address look-up itself is guarded by a mutex. */
+#define BSL6D_STATIC_SCRATCH_DOUBLES 262144
+BSL6D_API int bsl6d_density_static(const int32_t n[6], const double dv[3], const double* f, double* rho, void* stream,
+                         int* cuda_error);
 
 /* ---- odd stencil width, one displacement per point ------------------------------------------
  * PAPER.md:86-89 eq (6): for odd q the stencil stays centred on the grid point,

@@ -7,5 +7,5 @@ as hand-written sm_100a CUDA kernels behind a C ABI (include/bsl6d.h -> libbsl6d
 
 Importing this package does not load the shared library; the first call does, and raises if it is missing.
 """
-from .api import (Bsl6dError, Context, Grid, HostOp, LIB_PATH, Sweep, SYMBOLS, create, load_library, version,  # noqa: F401
-                  OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM)
+from .api import (Bsl6dError, Context, Grid, HostOp, LIB_PATH, Sweep, SYMBOLS, create, density_static, load_library,  # noqa: F401
+                  version, OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM, ESCRATCH, STATIC_SCRATCH_DOUBLES)

@@ -20,10 +20,13 @@ SYMBOLS = (
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_run_host_begin", "bsl6d_run_host_end", "bsl6d_advect_x1_peer", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
-    "bsl6d_advect_pointwise", "bsl6d_set_boundary",
+    "bsl6d_advect_pointwise", "bsl6d_set_boundary", "bsl6d_density_static",
 )
 
-OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
+OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM, ESCRATCH = 0, -1, -2, -3, -4, -5, -6
+
+#: doubles of scratch compiled into the library for density_static (BSL6D_STATIC_SCRATCH_DOUBLES, 2 MiB per GPU)
+STATIC_SCRATCH_DOUBLES = 262144
 
 
 class Grid(C.Structure):
@@ -69,6 +72,7 @@ def load_library() -> C.CDLL:
     lib.bsl6d_rotate.argtypes = [vp, dp, dp, C.POINTER(C.c_double), C.c_double, vp]
     lib.bsl6d_strang_step.argtypes = [vp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, vp]
     lib.bsl6d_density.argtypes = [vp, dp, dp, vp]
+    lib.bsl6d_density_static.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), dp, dp, vp, C.POINTER(C.c_int)]
     lib.bsl6d_run_host.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int]
     lib.bsl6d_run_host_begin.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int, C.c_int]
     lib.bsl6d_run_host_end.argtypes = [vp, C.c_int]
@@ -349,6 +353,41 @@ class Context:
 
 def create(n, lo, dx, degree) -> Context:
     return Context(n, lo, dx, degree)
+
+
+def density_static(n: Sequence[int], dv: Sequence[float], f, rho, stream=None):
+    """bsl6d_density_static: rho[x] = dv1*dv2*dv3 * sum_v f[x, v] without a context and without any allocation.
+
+    For users whose code may not allocate device memory while it runs -- a module inside an application that owns all
+    GPU memory through an allocator of its own, or a diagnostic between time steps that must not trigger the
+    synchronisation an allocation can bring.  The partial sums a long velocity block needs are kept in a 2 MiB array
+    compiled into the library (STATIC_SCRATCH_DOUBLES doubles; each GPU that loads the library holds it until the
+    process ends).  A grid that needs more raises Bsl6dError with code ESCRATCH.  The result has the same bits as
+    Context.density.  All calls on a GPU share that array: keep them on one stream or order them with events.  The
+    first call on a GPU looks the array's address up, so make it before you start capturing a stream.
+
+    n: the six extents; dv: spacings of v1, v2, v3; f: float64 CUDA tensor of shape n on the current device;
+    rho: float64 CUDA tensor with n[0]*n[1]*n[2] elements."""
+    lib = load_library()
+    n = [int(v) for v in n]
+    if len(n) != 6 or len(dv) != 3:
+        raise ValueError("n has six extents, dv three spacings")
+    if tuple(f.shape) != tuple(n):
+        raise ValueError(f"f: shape {tuple(f.shape)} != grid {tuple(n)}")
+    if rho.numel() != n[0] * n[1] * n[2]:
+        raise ValueError(f"rho: {rho.numel()} elements, want {n[0] * n[1] * n[2]}")
+    cn = (C.c_int32 * 6)(*n)
+    cdv = (C.c_double * 3)(*[float(v) for v in dv])
+    cuda_err = C.c_int(0)
+    rc = lib.bsl6d_density_static(cn, cdv, _dev_ptr(f, "f"), _dev_ptr(rho, "rho"), _stream(stream), C.byref(cuda_err))
+    if rc != OK:
+        detail = lib.bsl6d_strerror(rc).decode()
+        if rc == ECUDA:
+            detail += f"; cudaError {cuda_err.value}"
+        if rc == ESCRATCH:
+            detail += f" ({STATIC_SCRATCH_DOUBLES} doubles)"
+        raise Bsl6dError(rc, "bsl6d_density_static", detail)
+    return rho
 
 
 def version() -> int:

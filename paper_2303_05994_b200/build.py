@@ -30,6 +30,7 @@ UNITS = [
     ("bsl6d_ptile_q6.o", "bsl6d_ptile.cu", ["-DBSL6D_PTILE_Q=6"]),
     ("bsl6d_ptile_q8.o", "bsl6d_ptile.cu", ["-DBSL6D_PTILE_Q=8"]),
     ("bsl6d_ptile_q10.o", "bsl6d_ptile.cu", ["-DBSL6D_PTILE_Q=10"]),
+    ("bsl6d_static.o", "bsl6d_static.cu", []),
 ]
 HEADERS = ["sweep_kernels.cuh", "density_kernels.cuh", "fused_kernels.cuh", "fused_api.h", "field_kernels.cuh", "pointwise_kernels.cuh", "vblock_kernels.cuh", "ptile_kernels.cuh",
            os.path.join("..", "..", "include", "bsl6d.h")]

@@ -966,6 +966,7 @@ const char* bsl6d_strerror(int code) {
         case BSL6D_EUNSUPPORTED: return "unsupported configuration";
         case BSL6D_ECUDA: return "CUDA runtime error";
         case BSL6D_ENOMEM: return "out of memory";
+        case BSL6D_ESCRATCH: return "needs more scratch than the library's static device array holds";
         default: return "unknown error";
     }
 }
