@@ -16,7 +16,8 @@
  *
  * Ownership and execution
  *   Unless a function says HOST, every f / rho / shift-source pointer is a DEVICE pointer owned by the caller,
- *   8-byte aligned (16-byte for best speed); the library neither allocates nor frees them.  The context owns
+ *   8-byte aligned (16-byte for best speed: an f / f_tmp / f_out that is not on a 16-byte boundary runs without the
+ *   TMA-fed fused passes -- more passes, the same numbers); the library neither allocates nor frees them.  The context owns
  *   only small device tables.  Work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as
  *   void*, NULL = legacy default stream) and the call returns without synchronising.  Functions return 0 or
  *   a negative BSL6D_E* code; a failed call has enqueued nothing.  No exceptions, no printing, no aborts.
@@ -130,7 +131,8 @@ typedef struct bsl6d_sweep {
  * f_out (f_in == f_out is legal).  nsweeps <= 64; nsweeps == 0 copies. */
 BSL6D_API int bsl6d_advect_seq(bsl6d_ctx* ctx, const double* f_in, double* f_out, const bsl6d_sweep* sweeps,
                      int nsweeps, void* stream);
-/* Number of passes (kernel launches) bsl6d_advect_seq would use for this chain, or a negative error code. */
+/* Number of passes (kernel launches) bsl6d_advect_seq would use for this chain on 16-byte aligned arrays, or a
+ * negative error code. */
 BSL6D_API int bsl6d_seq_passes(bsl6d_ctx* ctx, const bsl6d_sweep* sweeps, int nsweeps);
 BSL6D_API int bsl6d_set_fusion(bsl6d_ctx* ctx, int enable);
 

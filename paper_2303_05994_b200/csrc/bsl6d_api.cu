@@ -589,7 +589,9 @@ bool try_vblock(const bsl6d_ctx* c, const SweepDesc* sw, int i, int cnt, Pass& p
     return true;
 }
 
-int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pass>& passes) {
+// tma_ok = false keeps the TMA-fed passes (persistent tile, whole-v-block) out of the plan: their tensor maps need
+// 16-byte aligned arrays, and the header only asks for 8.  Such chains run as round-1 tile passes or single sweeps.
+int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pass>& passes, bool tma_ok = true) {
     passes.clear();
     for (int i = 0; i < ns; ++i) {
         int rc = check_sweep_desc(c, sw[i]);
@@ -627,7 +629,7 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
             const double total = (by_count ? 1.0 : 0.7 + 0.13 * q) + best[i + 3];
             if (total < best[i] - eps) { best[i] = total; pick[i] = 3; }
         }
-        if (c->fusion && c->use_ptile) {
+        if (c->fusion && c->use_ptile && tma_ok) {
             for (int len = 2; len <= bsl6d::kMaxPSweeps && i + len <= ns; ++len) {
                 Pass p;
                 if (!try_ptile(c, sw, i, len, p)) break;      // a third dim (or the unit-stride dim) ends the chain
@@ -637,7 +639,7 @@ int plan_passes(const bsl6d_ctx* c, const SweepDesc* sw, int ns, std::vector<Pas
                 if (better(total, best[i])) { best[i] = total; pick[i] = 100 + len; candp[i] = p; }
             }
         }
-        if (c->fusion && c->use_vblock) {
+        if (c->fusion && c->use_vblock && tma_ok) {
             int run = 0;
             while (i + run < ns && sw[i + run].dim >= 3 && (c->fuse_all || sw[i + run].dim != 5) &&
                    run < bsl6d::kMaxVSweeps)
@@ -776,6 +778,9 @@ bool partial_overlap(const bsl6d_ctx* c, const void* x, const void* y) {
     return a < b + bytes && b < a + bytes;
 }
 
+// Both arrays on 16-byte boundaries (what a TMA tensor map needs)?  A null pointer counts as aligned.
+bool aligned16(const void* x, const void* y) { return (((uintptr_t)x | (uintptr_t)y) & 15u) == 0; }
+
 // f_in -> f_out: the first pass reads f_in and writes f_out, the others run in place on f_out.
 int run_sequence_in_out(bsl6d_ctx* c, const double* f_in, double* f_out, const SweepDesc* sw, int ns,
                         cudaStream_t st) {
@@ -784,7 +789,7 @@ int run_sequence_in_out(bsl6d_ctx* c, const double* f_in, double* f_out, const S
     std::vector<Pass> passes;
     int rc = check_device(c);
     if (rc) return rc;
-    rc = plan_passes(c, sw, ns, passes);
+    rc = plan_passes(c, sw, ns, passes, aligned16(f_in, f_out));
     if (rc) return rc;
     if (passes.empty()) {
         if (f_in != f_out) {
@@ -809,7 +814,7 @@ int run_sequence_pingpong(bsl6d_ctx* c, double* f, double* f_tmp, const SweepDes
     std::vector<Pass> passes;
     int rc = check_device(c);
     if (rc) return rc;
-    rc = plan_passes(c, sw, ns, passes);
+    rc = plan_passes(c, sw, ns, passes, aligned16(f, f_tmp));
     if (rc) return rc;
     const int np = (int)passes.size();
     double* cur = f;
@@ -1323,6 +1328,9 @@ int bsl6d_vp_step(bsl6d_ctx* c, double* f, double* f_tmp, double* rho, double* c
     if (!c || !f || !rho || !E || !E[0] || !E[1] || !E[2] || !std::isfinite(dt)) return BSL6D_EINVAL;
     if (closure != 0 && closure != 1) return BSL6D_EINVAL;
     if (!std::isfinite(c1) || !std::isfinite(e_fac)) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
+    // the field solve in the middle of the step needs a periodic x grid: say so before the first sweep is enqueued
+    if (c->open_x[0] || c->open_x[1] || c->open_x[2]) return BSL6D_EUNSUPPORTED;
     Shear sh[kMaxShears];
     int cnt = 0;
     if (B) {

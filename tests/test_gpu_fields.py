@@ -144,3 +144,11 @@ def test_field_error_paths():
             ctx.vp_step(f, None, rho, E, None, 0.1, 7, 1.0, 1.0)                 # unknown closure
         assert e.value.code == bsl.EINVAL
         assert ctx.launch_count() == 0
+        # an opened x dim (a slab with halo planes) has no spectral field solve: refused before anything is enqueued
+        ctx.set_boundary(0, 1)
+        f0 = f.clone()
+        with pytest.raises(bsl.Bsl6dError) as e:
+            ctx.vp_step(f, None, rho, E, None, 0.1, 0, 1.0, 1.0)
+        assert e.value.code == bsl.EUNSUPPORTED
+        torch.cuda.synchronize()
+        assert ctx.launch_count() == 0 and torch.equal(f, f0)

@@ -305,3 +305,46 @@ def test_tile_passes_with_displacements_of_many_cells(n, degree):
                 inp = fd.clone()
                 ctx.advect_seq(inp, inp, chain)
                 assert torch.equal(inp, single), (a, b, mode, "in place")
+
+
+@pytest.mark.parametrize("n,degree", [((8, 8, 8, 16, 16, 16), 7), ((4, 4, 4, 32, 32, 32), 9)])
+def test_arrays_on_8_byte_boundaries_run_without_tma_passes(n, degree):
+    """include/bsl6d.h allows f on an 8-byte boundary; a TMA tensor map needs 16.  The planner must then keep the
+    persistent-tile and v-block passes out of the plan instead of failing half way through a step: a Strang step, a
+    rotation and a chain on arrays offset by one double give, bit for bit, what the 16-byte aligned arrays give."""
+    _need_gpu()
+    w = wl.replace(wl.C5.reduced(n), degree=degree)
+    f = w.make_f("cuda")
+    Ed = [torch.from_numpy(e).cuda() for e in w.E()]
+    B = (0.0, 0.0, 1.0)
+
+    def odd(t=None):
+        """A copy of t (or an empty array of f's size) that starts one double past a 16-byte boundary."""
+        raw = torch.empty(f.numel() + 3, dtype=torch.float64, device="cuda")
+        off = 1 if raw.data_ptr() % 16 == 0 else 2
+        v = raw[off:off + f.numel()].view(f.shape)
+        assert v.data_ptr() % 16 == 8
+        if t is not None:
+            v.copy_(t)
+        return v
+
+    with bsl.create(w.n, w.lo, w.dx, w.degree) as ctx:
+        sw = six_sweeps(w, Ed)
+        want_step = ctx.strang_step(f.clone(), torch.empty_like(f), Ed, B, w.dt)
+        want_rot = ctx.rotate(f, torch.empty_like(f), B, w.dt)
+        want_seq = ctx.advect_seq(f, torch.empty_like(f), sw)
+        torch.cuda.synchronize()
+        got = odd(f)
+        ctx.strang_step(got, odd(), Ed, B, w.dt)               # both arrays misaligned, ping-pong
+        assert torch.equal(got, want_step)
+        got = odd(f)
+        ctx.strang_step(got, None, Ed, B, w.dt)                # in place
+        assert torch.equal(got, want_step)
+        got = f.clone()
+        ctx.strang_step(got, odd(), Ed, B, w.dt)               # only the second array misaligned
+        assert torch.equal(got, want_step)
+        assert torch.equal(ctx.rotate(odd(f), odd(), B, w.dt), want_rot)
+        assert torch.equal(ctx.rotate(f, odd(), B, w.dt), want_rot)
+        assert torch.equal(ctx.advect_seq(odd(f), odd(), sw), want_seq)
+        got = odd(f)
+        assert torch.equal(ctx.advect_seq(got, got, sw), want_seq)
