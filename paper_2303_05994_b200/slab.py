@@ -223,11 +223,9 @@ class Slab:
     def advect_x1(self, f_local: torch.Tensor, dt: float, max_check: bool = True):
         """x1 sweep over the whole local array, in place; interior results are exact, halo planes become stale."""
         if max_check:
-            vmax = max(abs(self.lo[3]), abs(self.lo[3] + (self.plan.n_global[3] - 1) * self.dx[3]))
-            need = self.plan.q // 2 + int(math.ceil(vmax * abs(dt) / self.dx[0]))
+            need = x1_planes_needed(self.lo, self.dx, self.plan.n_global, self.plan.q, dt)
             if need > self.plan.w:
-                raise ValueError(f"displacement of {vmax * abs(dt) / self.dx[0]:.2f} cells needs {need} halo planes, "
-                                 f"the slab has {self.plan.w}")
+                raise ValueError(f"a step of dt={dt:g} needs {need} halo planes, the slab has {self.plan.w}")
         self.ctx_x1.advect(f_local, f_local, 0, None, dt)
 
     def advect(self, f_local: torch.Tensor, dim: int, shift_source, dt: float):
@@ -314,6 +312,13 @@ class Slab:
         return h
 
 
+def x1_planes_needed(lo, dx, n_global, q: int, dt: float) -> int:
+    """Planes of a neighbour an x1 sweep of length dt can reach: half the stencil plus the largest displacement
+    |v1| * |dt| / dx1 over the v1 nodes, rounded up (include/bsl6d.h, bsl6d_set_boundary / bsl6d_advect_x1_peer)."""
+    vmax = max(abs(lo[3]), abs(lo[3] + (n_global[3] - 1) * dx[3]))
+    return q // 2 + int(math.ceil(vmax * abs(dt) / dx[0]))
+
+
 # ---- slabs WITHOUT halo planes: the x1 sweep reads the neighbours' planes through peer memory -------------------------
 class PeerSlab:
     """One rank's slab as two plain arrays of L planes (ping-pong); the x1 sweep (bsl6d_advect_x1_peer) reads the w
@@ -351,7 +356,14 @@ class PeerSlab:
     def destroy(self):
         self.ctx.destroy()
 
-    def advect_x1(self, dt: float):
+    def advect_x1(self, dt: float, max_check: bool = True):
+        """The x1 sweep over peer memory.  The slab was planned for a largest displacement: a longer step would make the
+        kernel read beyond the w neighbour planes it is promised (zeros, silently), so it is refused here."""
+        if max_check:
+            need = x1_planes_needed(self.lo, self.dx, self.plan.n_global, self.plan.q, dt)
+            if need > self.plan.w or need > self.plan.L:
+                raise ValueError(f"a step of dt={dt:g} needs {need} neighbour planes, the slab was planned for "
+                                 f"{self.plan.w} (thickness {self.plan.L})")
         c = self.cur
         self.ctx.advect_x1_peer(self.buf[c], self.left[c], self.right[c], self.buf[1 - c], self.plan.w, None, dt)
         self.cur = 1 - c

@@ -38,6 +38,21 @@ def _gather(ss):
     return torch.cat([s.f for s in ss], dim=0)
 
 
+def test_x1_peer_sweep_refuses_a_step_longer_than_planned():
+    """A dt above the one the slab was planned for would read beyond the promised neighbour planes (silently zeros)."""
+    _need_gpu()
+    w = wl.C2.reduced((32, 4, 2, 8, 4, 8))
+    f = w.make_f("cuda")
+    ss = _ring(w, 2, 0.5, f)                                    # planned for half a cell
+    before = ss[0].ctx.launch_count()
+    with pytest.raises(ValueError):
+        ss[0].advect_x1(1.7 * w.dx[0] / 6.0)                    # 1.7 cells
+    assert ss[0].ctx.launch_count() == before and ss[0].cur == 0
+    ss[0].advect_x1(0.4 * w.dx[0] / 6.0)                        # within the plan
+    for s in ss:
+        s.destroy()
+
+
 @pytest.mark.parametrize("world", (1, 2, 4))
 @pytest.mark.parametrize("dt_cells", (0.37, 2.3, "whole"))
 def test_x1_peer_sweep_equals_undivided(world, dt_cells):

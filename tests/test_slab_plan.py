@@ -30,6 +30,22 @@ def test_plan_geometry():
     assert (one.left, one.right, one.w, one.L) == (0, 0, 2, 8)
 
 
+def test_planes_needed_by_an_x1_sweep():
+    """Half the stencil plus the largest |v1| dt / dx1, rounded up -- what both slab forms check before an x1 sweep."""
+    n = (32, 4, 4, 8, 8, 8)
+    lo = (0.0, 0.0, 0.0, -6.0, -6.0, -6.0)
+    dx = (0.25, 1.0, 1.0, 1.5, 1.5, 1.5)                          # v1 nodes -6 .. 4.5: |v1| <= 6
+    assert slab.x1_planes_needed(lo, dx, n, 8, 0.0) == 4
+    assert slab.x1_planes_needed(lo, dx, n, 8, 0.01) == 5         # 0.24 cells
+    assert slab.x1_planes_needed(lo, dx, n, 8, -0.1) == 4 + 3     # 2.4 cells, the sign of dt does not matter
+    assert slab.x1_planes_needed(lo, dx, n, 6, 0.125) == 3 + 3    # exactly 3 cells
+    lo2 = (0.0, 0.0, 0.0, -3.0, -6.0, -6.0)                       # v1 nodes -3 .. 7.5: the upper end decides
+    assert slab.x1_planes_needed(lo2, dx, n, 8, 0.1) == 4 + 3
+    # consistent with the plan: a slab planned for that displacement accepts the step
+    p = slab.plan_slab(n, 7, 2, 0, 6.0 * 0.1 / 0.25)
+    assert slab.x1_planes_needed(lo, dx, n, p.q, 0.1) == p.w
+
+
 def test_plan_rejects_what_the_halo_cannot_serve():
     with pytest.raises(ValueError):
         slab.plan_slab((30, 4, 4, 8, 8, 8), 7, 4, 0, 1.0)     # 30 planes do not divide among 4 ranks (PAPER.md:148)
