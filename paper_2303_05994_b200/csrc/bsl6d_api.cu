@@ -74,10 +74,6 @@ struct KernelChoice {
 
 // Launch shape of the strided sweep: T threads per block, at least MINB resident blocks per SM (caps the
 // registers ptxas may use: a thread holds its whole pencil, 2*(N [+Q-1]) registers, plus 2*Q for the weights).
-#ifdef BSL6D_TUNE_T
-template <int N, int Q, bool P> constexpr int strided_threads() { return BSL6D_TUNE_T; }
-template <int N, int Q, bool P> constexpr int strided_minblocks() { return BSL6D_TUNE_MINB; }
-#else
 // Pencils that fit 128 registers: 4 blocks of 128 threads (16 warps/SM).  Longer pencils (N = 48 with Q = 10, N = 64)
 // allow only ~12 warps/SM; they run as blocks of 64 threads, 6 (or 4) per SM.  Measured against 3 blocks of 128
 // threads in alternating runs on one box: no difference beyond noise (C5 x sweeps 6.21-6.48 TB/s either way) -- inside a
@@ -85,42 +81,29 @@ template <int N, int Q, bool P> constexpr int strided_minblocks() { return BSL6D
 // four threads per pencil (S > 1 below) were slower (6.09 / 5.0-5.6 TB/s): the shared rows are re-read through L1/L2.
 template <int N, int Q, bool P>
 constexpr int strided_regs_wanted() { return 2 * (N + (P ? 0 : Q - 1)) + 2 * Q + 24; }
-#ifndef BSL6D_TUNE_LONG_T
-#define BSL6D_TUNE_LONG_T 64
-#define BSL6D_TUNE_LONG_MINB 6
-#endif
+constexpr auto kTuneLongT = 64;
+constexpr auto kTuneLongMinb = 6;
 template <int N, int Q, bool P>
-constexpr int strided_threads() { return strided_regs_wanted<N, Q, P>() <= 128 ? 128 : BSL6D_TUNE_LONG_T; }
+constexpr int strided_threads() { return strided_regs_wanted<N, Q, P>() <= 128 ? 128 : kTuneLongT; }
 template <int N, int Q, bool P>
 constexpr int strided_minblocks() {
     constexpr int est = strided_regs_wanted<N, Q, P>();
-    return est <= 128 ? 4 : (est <= 176 ? BSL6D_TUNE_LONG_MINB : (BSL6D_TUNE_LONG_MINB * 2) / 3);
+    return est <= 128 ? 4 : (est <= 176 ? kTuneLongMinb : (kTuneLongMinb * 2) / 3);
 }
-#endif
 
 // Segments per pencil: 1 (a thread owns its whole pencil) unless the pencil is too long for 4 blocks per SM.
-#ifdef BSL6D_TUNE_SS
-template <int N, int Q, bool P> constexpr int strided_segments() { return (N >= 48 && N % BSL6D_TUNE_SS == 0 && N / BSL6D_TUNE_SS >= Q) ? BSL6D_TUNE_SS : 1; }
-#else
 template <int N, int Q, bool P> constexpr int strided_segments() { return 1; }
-#endif
 
 template <int N, int Q, bool P>
 KernelChoice strided_choice() {
     constexpr int S = strided_segments<N, Q, P>();
     constexpr int T = strided_threads<N, Q, P>();
-#ifdef BSL6D_TUNE_SMINB
-    constexpr int MINB = S == 1 ? strided_minblocks<N, Q, P>() : BSL6D_TUNE_SMINB;
-#else
     constexpr int MINB = S == 1 ? strided_minblocks<N, Q, P>() : 4;
-#endif
     // Out of place, long periodic pencils stream through a register window instead (sweep_stream_kernel: 96-122 instead
     // of 162-168 registers at N = 48, Q = 10; C5 x sweeps +1.7-2.8 % in alternating runs on one box).  Zero-extended
     // long pencils (N = 64, Q = 6) and the pencils that fit 128 registers anyway measured 0.6-2 % slower that way.
-#ifndef BSL6D_TUNE_STREAM_REGS
-#define BSL6D_TUNE_STREAM_REGS 128
-#endif
-    if constexpr (P && S == 1 && strided_regs_wanted<N, Q, P>() > BSL6D_TUNE_STREAM_REGS) {
+constexpr auto kTuneStreamRegs = 128;
+    if constexpr (P && S == 1 && strided_regs_wanted<N, Q, P>() > kTuneStreamRegs) {
         KernelChoice kc{bsl6d::sweep_strided_kernel<N, Q, P, T, MINB, S>, T, 0, 0, S};
         kc.fn_oop = bsl6d::sweep_stream_kernel<N, Q, P, 128, 4, 12>;
         kc.oop_threads = 128;
@@ -130,21 +113,12 @@ KernelChoice strided_choice() {
 }
 
 // Launch shape of the unit-stride sweep: S segments per pencil, T threads (a multiple of 32*S), MINB blocks/SM.
-#ifdef BSL6D_TUNE_US
-template <int N, int Q> constexpr int unit_segments() { return (N % BSL6D_TUNE_US == 0) ? BSL6D_TUNE_US : 1; }
-template <int N, int Q> constexpr int unit_minblocks() { return BSL6D_TUNE_UMINB; }
-#else
 template <int N, int Q> constexpr int unit_segments() { return N >= 48 ? 4 : 1; }
 template <int N, int Q> constexpr int unit_minblocks() { return (N >= 48 && Q <= 8) ? 6 : 4; }   // q = 10 at 80 registers spills
-#endif
 // Tile filled by cp.async (true) or by loads staged in registers.  Alternating runs on one box, v3 sweep in-step, GB/s:
 // C3 (N = 64, q = 6, with 6 blocks/SM) 6440-6486 -> 6915-6948; C2 (N = 32, q = 8) 6631-6668 -> 6946-7009;
 // C5 (N = 32, q = 10) 6715 -> 6600-6612, so the widest stencil on short pencils keeps the register fill.
-#ifdef BSL6D_TUNE_UASYNC
-template <int N, int Q> constexpr bool unit_async() { return BSL6D_TUNE_UASYNC != 0; }
-#else
 template <int N, int Q> constexpr bool unit_async() { return unit_segments<N, Q>() > 1 || Q <= 8; }
-#endif
 template <int N, int Q> constexpr int unit_threads() { return 128 % (32 * unit_segments<N, Q>()) == 0 ? 128 : 32 * unit_segments<N, Q>(); }
 
 template <int N, int Q>

@@ -14,11 +14,7 @@ constexpr int Q = BSL6D_FUSED_Q;
 constexpr int cgcd(int a, int b) { return b == 0 ? a : cgcd(b, a % b); }
 
 // Tile shape policy: C = 8 contiguous doubles (64 B segments) while the tile stays <= ~100 KB, else 4.
-#ifdef BSL6D_TUNE_FC
-template <int NA, int NB> constexpr int fused_C() { return BSL6D_TUNE_FC; }
-#else
 template <int NA, int NB> constexpr int fused_C() { return NA * NB <= 1536 ? 8 : 4; }
-#endif
 
 template <int NA, int NB, bool PA, bool PB, int PAT>
 constexpr int fused_minblocks() {

@@ -12,40 +12,26 @@ namespace {
 // segments, 4 blocks per SM: 9.0 / 10.5 / 10.2 / 10.1).  A shared-memory tile variant of the strided kernel (same
 // structure as the unit-stride one, rows of 32 or 64 pencils) was measured too: no better than the register kernel
 // (q = 9: 12.5-13.6 against 11.9-12.4 ms) and dropped.
-#ifndef BSL6D_TUNE_PWT
-#define BSL6D_TUNE_PWT 128
-#endif
-#ifndef BSL6D_TUNE_PWD7
-#define BSL6D_TUNE_PWD7 12
-#endif
-#ifndef BSL6D_TUNE_PWM7
-#define BSL6D_TUNE_PWM7 3
-#endif
-#ifndef BSL6D_TUNE_PWD9
-#define BSL6D_TUNE_PWD9 4
-#endif
-#ifndef BSL6D_TUNE_PWM9
-#define BSL6D_TUNE_PWM9 5
-#endif
-#ifndef BSL6D_TUNE_PWMINB
-#define BSL6D_TUNE_PWMINB 6
-#endif
-#ifndef BSL6D_TUNE_PWPB
-#define BSL6D_TUNE_PWPB 32
-#endif
+constexpr auto kTunePwt = 128;
+constexpr auto kTunePwd7 = 12;
+constexpr auto kTunePwm7 = 3;
+constexpr auto kTunePwd9 = 4;
+constexpr auto kTunePwm9 = 5;
+constexpr auto kTunePwminb = 6;
+constexpr auto kTunePwpb = 32;
 
-template <int Q> constexpr int pw_lookahead() { return Q >= 9 ? BSL6D_TUNE_PWD9 : (Q >= 7 ? BSL6D_TUNE_PWD7 : 8); }
-template <int Q> constexpr int pw_minblocks() { return Q >= 9 ? BSL6D_TUNE_PWM9 : (Q >= 7 ? BSL6D_TUNE_PWM7 : 4); }
+template <int Q> constexpr int pw_lookahead() { return Q >= 9 ? kTunePwd9 : (Q >= 7 ? kTunePwd7 : 8); }
+template <int Q> constexpr int pw_minblocks() { return Q >= 9 ? kTunePwm9 : (Q >= 7 ? kTunePwm7 : 4); }
 
 template <int N, int Q>
 bool by_kind(bool periodic, bool unit, PointwiseChoice& c) {
-    constexpr int T = BSL6D_TUNE_PWT, D = pw_lookahead<Q>(), MB = pw_minblocks<Q>();
+    constexpr int T = kTunePwt, D = pw_lookahead<Q>(), MB = pw_minblocks<Q>();
     c = PointwiseChoice{};
     if (unit) {
         if (periodic) return false;
-        constexpr int S = N >= 48 ? 8 : (N >= 16 ? 4 : 1), PB = BSL6D_TUNE_PWPB;      // PB pencils x S segments per block
+        constexpr int S = N >= 48 ? 8 : (N >= 16 ? 4 : 1), PB = kTunePwpb;      // PB pencils x S segments per block
         constexpr size_t smem = 2 * sizeof(double) * PB * (N | 1);
-        constexpr int MINB = S == 1 ? 8 : (S == 8 ? 3 : BSL6D_TUNE_PWMINB);
+        constexpr int MINB = S == 1 ? 8 : (S == 8 ? 3 : kTunePwminb);
         c.fn = (const void*)pointwise_unit_kernel<N, Q, S, PB, MINB>;
         c.threads = PB * S;
         c.smem = smem;
@@ -105,7 +91,6 @@ bool generic_by_q(int n, int q, bool periodic, bool unit, PointwiseChoice& c) {
 }  // namespace
 
 bool pointwise_lookup(int n, int q, bool periodic, bool unit_stride, PointwiseChoice& out) {
-#ifndef BSL6D_TUNE_PWGENERIC
     {
         bool ok = false;
         switch (n) {
@@ -119,7 +104,6 @@ bool pointwise_lookup(int n, int q, bool periodic, bool unit_stride, PointwiseCh
         }
         if (ok) return true;
     }
-#endif
     return generic_by_q(n, q, periodic, unit_stride, out);
 }
 

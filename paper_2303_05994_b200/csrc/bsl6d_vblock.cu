@@ -44,14 +44,12 @@ bool make_map(CUtensorMap* m, const double* f, uint32_t nx, int nv, int cw) {
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-#ifndef BSL6D_TUNE_V3PATH
-#define BSL6D_TUNE_V3PATH kV3ViaL2
-#endif
+constexpr auto kTuneV3path = kV3ViaL2;
 
 template <int NV, int Q, int CL, int MINB>
 VBlockChoice choice() {
     using G = VBlockGeom<NV, CL>;
-    return VBlockChoice{(const void*)vblock_kernel<NV, Q, CL, MINB, BSL6D_TUNE_V3PATH>, G::T, G::kSmemBytes, CL, G::CW};
+    return VBlockChoice{(const void*)vblock_kernel<NV, Q, CL, MINB, kTuneV3path>, G::T, G::kSmemBytes, CL, G::CW};
 }
 
 // The other cut of the same block: box = [1][nv/cl j1-planes][nv][16 doubles], 128-byte half rows, 128B swizzle.
@@ -67,19 +65,15 @@ bool make_map_b(CUtensorMap* m, const double* f, uint32_t nx, int nv, int cl) {
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-#ifndef BSL6D_TUNE_VCL
-#define BSL6D_TUNE_VCL 4
-#endif
-#ifndef BSL6D_TUNE_VMINB
-#define BSL6D_TUNE_VMINB 2
-#endif
+constexpr auto kTuneVcl = 4;
+constexpr auto kTuneVminb = 2;
 
 template <int Q>
 bool by_nv(int nv, VBlockChoice& out) {
     switch (nv) {
         case 8: out = choice<8, Q, 1, 4>(); return true;
         case 16: out = choice<16, Q, 1, 3>(); return true;
-        case 32: out = choice<32, Q, BSL6D_TUNE_VCL, BSL6D_TUNE_VMINB>(); return true;
+        case 32: out = choice<32, Q, kTuneVcl, kTuneVminb>(); return true;
         default: return false;
     }
 }

@@ -23,15 +23,9 @@
 
 #include "sweep_kernels.cuh"
 
-#ifndef BSL6D_PTILE_ROT
-#define BSL6D_PTILE_ROT 1
-#endif
-#ifndef BSL6D_PTILE_STREAM
-#define BSL6D_PTILE_STREAM 1          // zero-extended pencils: stream through a register window where that is safe
-#endif
-#ifndef BSL6D_PTILE_STREAM_D
-#define BSL6D_PTILE_STREAM_D 4
-#endif
+constexpr auto kPtileRot = 1;
+constexpr auto kPtileStream = 1;          // zero-extended pencils: stream through a register window where that is safe
+constexpr auto kPtileStreamD = 4;
 
 namespace bsl6d {
 
@@ -144,7 +138,7 @@ __device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, doub
         kc = kc > (long long)(2 * N + 2 * Q) ? (long long)(2 * N + 2 * Q) : kc;
         const int r0 = (int)kc + (1 - Q / 2);
         rot = par < 0 ? 0 : ((r0 + par) & 1);
-        if (BSL6D_PTILE_STREAM && r0 > -Q) {
+        if (kPtileStream && r0 > -Q) {
             // Streaming form (ncu: in the all-loads-first form below the fp64 pipe is the top stall of a pass and yet
             // only half busy -- every warp alternates a burst of shared-memory loads with a burst of DFMAs).  Rows are
             // read in increasing order, D outputs ahead of their first use, and output j (row j + rot) is stored as
@@ -153,7 +147,7 @@ __device__ __forceinline__ void pencil_in_place(uint32_t base, double sval, doub
             // first.  Same values, same order of operations per output: bit-identical to the form below.
             // Measured (alternating runs, ms): v1+v2 at C5 10.57 -> 10.27, three shears at C2 3.84 -> 3.75, Strang step
             // at C2 23.1 -> 22.6; look-ahead 2 or 8 instead of 4: no better.
-            constexpr int D = BSL6D_PTILE_STREAM_D;
+            constexpr int D = kPtileStreamD;
             auto ld = [&](int t) -> double {
                 int tt = t + rot;
                 if (tt >= NU) tt -= NU;
@@ -316,7 +310,7 @@ __global__ void __launch_bounds__((PTileGeom<NA, NB>::THREADS), 1)
                 for (int p = gt; p < NA * C; p += GT) {
                     const uint32_t ia = (uint32_t)p / C, c = (uint32_t)p % C;
                     const double sval = p == gt ? sval_first : shift_source(s, p);
-                    pt::pencil_in_place<NB, Q, PB, (uint32_t)ROW>(buf + ia * (uint32_t)PLANE + c * 8u, sval, sw.scale, (BSL6D_PTILE_ROT && !PA) ? (int)(ia & 1u) : -1);
+                    pt::pencil_in_place<NB, Q, PB, (uint32_t)ROW>(buf + ia * (uint32_t)PLANE + c * 8u, sval, sw.scale, (kPtileRot && !PA) ? (int)(ia & 1u) : -1);
                 }
             }
             pt::group_sync(1 + g, GT);
