@@ -23,9 +23,13 @@
  *   a negative BSL6D_E* code; a failed call has enqueued nothing.  No exceptions, no printing, no aborts.
  *   There is no CPU fallback anywhere: without a CUDA device bsl6d_create fails with BSL6D_ECUDA.
  *   Preconditions not checked: f finite; |displacement| < 2^30 cells.
+ *   Size limits (32-bit index arithmetic in the kernels): a sweep along dim d needs (number of pencils) =
+ *   npts / n[d] < 2^32, else BSL6D_EUNSUPPORTED; the fused passes need npts = n0*..*n5 <= 2^32 - 1 -- a larger grid
+ *   (48^6 = 98 GB would still fit one B200) is NOT refused: every chain then runs as single sweeps, correct but with
+ *   one pass per sweep, and bsl6d_seq_passes reports that count.  bsl6d_density needs n0*n1*n2 * G < 2^31.
  *   A context is not thread-safe: one host thread at a time per context.  Sweeps and rotations of one context may be in
- *   flight on several streams; bsl6d_density with v-blocks above 32768 points, bsl6d_field_* and bsl6d_vp_step use work
- *   arrays of the context and must not overlap each other in time; each bsl6d_run_host slot is one queue with work
+ *   flight on several streams; bsl6d_density with v-blocks above 32768 points (bsl6d_density_scratch lifts that),
+ *   bsl6d_field_* and bsl6d_vp_step use work arrays of the context and must not overlap each other in time; each bsl6d_run_host slot is one queue with work
  *   arrays of its own.
  */
 #ifndef BSL6D_H
@@ -173,6 +177,13 @@ BSL6D_API int bsl6d_advect_x1_peer(bsl6d_ctx* ctx, const double* f_in, const dou
 /* Density moment rho[x] = dv1*dv2*dv3 * sum_{j1,j2,j3} f[x, j]   (eq (2); bare moment, reading S9).
  * rho: n0*n1*n2 doubles.  The summation order is fixed (deterministic, tree-shaped). */
 BSL6D_API int bsl6d_density(bsl6d_ctx* ctx, const double* f, double* rho, void* stream);
+/* The same moment with the work array given by the caller, so that several moments of one context can be in flight on
+ * different streams at once (bsl6d_density keeps the partial sums of split v-blocks in ONE array of the context; two
+ * overlapping calls race on it).  scratch: DEVICE, bsl6d_density_scratch_doubles(ctx) doubles = n0*n1*n2 * G when a
+ * v-block is cut into G > 1 chunks of <= 32768 doubles, else 0 (scratch may then be NULL).  One scratch array per
+ * stream in flight; contents on entry do not matter.  Same bits as bsl6d_density. */
+BSL6D_API int bsl6d_density_scratch(bsl6d_ctx* ctx, const double* f, double* rho, double* scratch, void* stream);
+BSL6D_API long long bsl6d_density_scratch_doubles(const bsl6d_ctx* ctx);
 
 /* ---- the density moment without any allocation ----------------------------------------------------------------
  * For callers that may not call cudaMalloc / cudaFree (or anything that does): code living inside a host application

@@ -20,7 +20,8 @@ SYMBOLS = (
     "bsl6d_strang_step", "bsl6d_density", "bsl6d_run_host", "bsl6d_run_host_begin", "bsl6d_run_host_end", "bsl6d_advect_x1_peer", "bsl6d_strerror", "bsl6d_last_cuda_error",
     "bsl6d_launch_count", "bsl6d_kernel_name", "bsl6d_version", "bsl6d_advect_seq", "bsl6d_seq_passes",
     "bsl6d_set_fusion", "bsl6d_field_poisson", "bsl6d_field_adiabatic", "bsl6d_vp_step",
-    "bsl6d_advect_pointwise", "bsl6d_set_boundary", "bsl6d_density_static",
+    "bsl6d_advect_pointwise", "bsl6d_set_boundary", "bsl6d_density_static", "bsl6d_density_scratch",
+    "bsl6d_density_scratch_doubles",
 )
 
 OK, EINVAL, EALIAS, EUNSUPPORTED, ECUDA, ENOMEM, ESCRATCH = 0, -1, -2, -3, -4, -5, -6
@@ -72,6 +73,9 @@ def load_library() -> C.CDLL:
     lib.bsl6d_rotate.argtypes = [vp, dp, dp, C.POINTER(C.c_double), C.c_double, vp]
     lib.bsl6d_strang_step.argtypes = [vp, dp, dp, C.POINTER(C.c_void_p), C.POINTER(C.c_double), C.c_double, vp]
     lib.bsl6d_density.argtypes = [vp, dp, dp, vp]
+    lib.bsl6d_density_scratch.argtypes = [vp, dp, dp, dp, vp]
+    lib.bsl6d_density_scratch_doubles.argtypes = [vp]
+    lib.bsl6d_density_scratch_doubles.restype = C.c_longlong
     lib.bsl6d_density_static.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), dp, dp, vp, C.POINTER(C.c_int)]
     lib.bsl6d_run_host.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int]
     lib.bsl6d_run_host_begin.argtypes = [vp, dp, dp, C.POINTER(HostOp), C.c_int, C.c_int]
@@ -306,6 +310,19 @@ class Context:
         self._shape_ok(f, "f"); self._count_ok(rho, self.nx, "rho")
         self._check(self._lib.bsl6d_density(self._h, _dev_ptr(f, "f"), _dev_ptr(rho, "rho"), _stream(stream)),
                     "bsl6d_density")
+        return rho
+
+    def density_scratch_doubles(self) -> int:
+        return int(self._lib.bsl6d_density_scratch_doubles(self._h))
+
+    def density_scratch(self, f, rho, scratch, stream=None):
+        """bsl6d_density_scratch: the moment with a caller-owned work array (one per stream in flight)."""
+        self._shape_ok(f, "f"); self._count_ok(rho, self.nx, "rho")
+        need = self.density_scratch_doubles()
+        if need and (scratch is None or scratch.numel() < need):
+            raise ValueError(f"scratch: want {need} doubles")
+        self._check(self._lib.bsl6d_density_scratch(self._h, _dev_ptr(f, "f"), _dev_ptr(rho, "rho"),
+                                                    _dev_ptr(scratch, "scratch"), _stream(stream)), "bsl6d_density_scratch")
         return rho
 
     def _host_ops(self, ops: Sequence[dict]):

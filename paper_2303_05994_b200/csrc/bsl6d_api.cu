@@ -1347,6 +1347,18 @@ int bsl6d_density(bsl6d_ctx* c, const double* f, double* rho, void* stream) {
     return density_impl(c, f, rho, c->d_part, stream);
 }
 
+int bsl6d_density_scratch(bsl6d_ctx* c, const double* f, double* rho, double* scratch, void* stream) {
+    if (!c || !f || !rho || (c->dens_G > 1 && !scratch)) return BSL6D_EINVAL;
+    if (int rcd = check_device(c)) return rcd;
+    return density_impl(c, f, rho, scratch, stream);
+}
+
+long long bsl6d_density_scratch_doubles(const bsl6d_ctx* c) {
+    if (!c) return BSL6D_EINVAL;
+    if (c->dens_G <= 1) return 0;
+    return (long long)((size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * c->dens_G);
+}
+
 // part: nx * G doubles of scratch for the partial sums of split v-blocks (unused when G == 1)
 static int density_impl(bsl6d_ctx* c, const double* f, double* rho, double* part, void* stream) {
     const bsl6d_grid& g = c->g;

@@ -466,3 +466,39 @@ def test_error_codes():
             ctx.rotate(a, a, [30.0, 40.0, 0.0], 0.2)          # oblique B, more than a full turn
         assert e.value.code == bsl.EUNSUPPORTED
         assert ctx.launch_count() == 0                        # failed calls enqueue nothing
+
+
+def test_density_with_caller_scratch_on_two_streams():
+    """bsl6d_density_scratch: two moments of ONE context in flight on two streams, each with a work array of its own,
+    give the bits of bsl6d_density (whose single work array two overlapping calls would race on)."""
+    _need_gpu()
+    n = (6, 4, 4, 64, 32, 40)                                  # v-block of 81920 points: 3 chunks per x-point
+    w = mini(n, 7, seed=12, kind="maxwell_x1")
+    f1 = dev(w.make_f("cpu").numpy())
+    f2 = (f1 * 1.5 + 0.25).contiguous()
+    with ctx_for(w) as ctx:
+        need = ctx.density_scratch_doubles()
+        assert need == 6 * 4 * 4 * 3
+        want1 = ctx.density(f1, torch.empty(n[:3], dtype=torch.float64, device="cuda")).clone()
+        want2 = ctx.density(f2, torch.empty(n[:3], dtype=torch.float64, device="cuda")).clone()
+        torch.cuda.synchronize()
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        w1 = torch.full((need,), float("nan"), dtype=torch.float64, device="cuda")
+        w2 = torch.full((need,), float("nan"), dtype=torch.float64, device="cuda")
+        r1 = torch.empty(n[:3], dtype=torch.float64, device="cuda")
+        r2 = torch.empty(n[:3], dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(20):                                   # interleaved launches on the two streams
+            ctx.density_scratch(f1, r1, w1, stream=s1)
+            ctx.density_scratch(f2, r2, w2, stream=s2)
+        torch.cuda.synchronize()
+        assert torch.equal(r1, want1) and torch.equal(r2, want2)
+        with pytest.raises(ValueError):
+            ctx.density_scratch(f1, r1, None)
+    small = mini((3, 2, 4, 5, 6, 7), 7, seed=11, kind="maxwell_x1")   # one chunk: no work array needed
+    fs = dev(small.make_f("cpu").numpy())
+    with ctx_for(small) as ctx:
+        assert ctx.density_scratch_doubles() == 0
+        a = ctx.density_scratch(fs, torch.empty(small.n[:3], dtype=torch.float64, device="cuda"), None)
+        b = ctx.density(fs, torch.empty(small.n[:3], dtype=torch.float64, device="cuda"))
+        assert torch.equal(a, b)
