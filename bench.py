@@ -70,6 +70,9 @@ def parse_args():
     p.add_argument("--peer", action="store_true",
                    help="with --sharded: slabs WITHOUT halo planes -- the x1 sweep reads the neighbours' planes through "
                         "peer memory (bsl6d_advect_x1_peer; CUDA IPC between the ranks), no exchange step")
+    p.add_argument("--link-benchmark", action="store_true",
+                   help="host link yardstick for the e2e leg: pinned H2D alone, D2H alone and both at once "
+                        "(one cudaMemcpyAsync per direction per repetition); prints one JSON line")
     p.add_argument("--paper-benchmark", action="store_true",
                    help="instead of the contract step: the paper's own section-5 benchmark (37^6, random per-point "
                         "shifts, odd widths 3/5/7/9, every direction) through bsl6d_advect_pointwise")
@@ -681,25 +684,36 @@ def measure_e2e(G: Gpu, w, f0_host, K: int):
             out = torch.empty(w.n, dtype=torch.float64, pin_memory=True)
             outs = [out, out]
             hops2 = [hops, make_ops()[0]]
-            kp = max(4, 2 * ke)
+            # eight or more steps: with four, filling and draining the two-deep pipeline (one upload without a download
+            # beside it, one download without an upload) is a third of the timed region
+            kp = max(8, 2 * ke)
             for sl in (0, 1):                                     # warm-up: allocates the second slot's device buffer
                 ctx.run_host_begin(f0_host, outs[sl], hops2[sl], sl)
             ctx.run_host_end(0)
             ctx.run_host_end(1)
             G.barrier()
             t0 = time.perf_counter()
+            t_done = []                                           # host time at which step k's result was complete
             for k in range(kp):
                 sl = k & 1
                 if k >= 2:
                     ctx.run_host_end(sl)                          # the step that used this slot's buffers is complete
+                    t_done.append(time.perf_counter())
                 ctx.run_host_begin(f0_host, outs[sl], hops2[sl], sl)
             ctx.run_host_end(0)
+            t_done.append(time.perf_counter())
             ctx.run_host_end(1)
+            t_done.append(time.perf_counter())
             tp = max_over_ranks(time.perf_counter() - t0, G.dev)
+            steady = max_over_ranks((t_done[-1] - t_done[1]) / (kp - 2), G.dev)
             rec.update({"value": whole_job_value(w.npts, n_sweeps(w), kp, G.world, 1e3 * tp), "steps": kp,
                         "ms_per_step": 1e3 * tp / kp,
                         "api": "bsl6d_run_host_begin / bsl6d_run_host_end, two steps in flight (pinned host buffers): "
                                "the upload of step k+1 overlaps the download of step k",
+                        "steady_ms_per_step": 1e3 * steady,
+                        "steady_note": "completion-to-completion time per step from the second step on (pipeline full); "
+                                       "`value` and `ms_per_step` are over the whole timed region, fill and drain "
+                                       "included; `python bench.py --link-benchmark` gives the link's own floor",
                         "serial": serial})
             del outs, out
         except Exception as exc:                              # e.g. the pinned allocation failed: keep the serial figure
@@ -926,6 +940,66 @@ def run_sharded_peer(args, w):
         G.dist.destroy_process_group()
 
 
+def run_link_benchmark(args):
+    """What the host link gives the e2e leg at best: one pinned buffer each way (4 GiB, or what the box allows), copied
+    with ONE cudaMemcpyAsync per direction per repetition (torch copy_ non_blocking), alone and with both directions in
+    flight on two streams.  The e2e step moves 8*npts bytes up and 8*npts bytes down, so its floor is
+    8*npts / duplex rate; bench.py's e2e figure is to be read against that."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    nbytes = 4 << 30
+    while nbytes > (256 << 20) and not host_memory_allows(2 * nbytes, factor=1.5):
+        nbytes >>= 1
+    n = nbytes // 8
+    h_up = torch.empty(n, dtype=torch.float64, pin_memory=True).fill_(1.0)
+    h_dn = torch.empty(n, dtype=torch.float64, pin_memory=True)
+    d_up = torch.empty(n, dtype=torch.float64, device="cuda")
+    d_dn = torch.ones(n, dtype=torch.float64, device="cuda")
+    s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+    reps = max(3, args.steps if args.steps else 5)
+
+    def timed(up: bool, dn: bool):
+        torch.cuda.synchronize()
+        ev = {k: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for k in ("up", "dn")}
+        t0 = time.perf_counter()
+        if up:
+            with torch.cuda.stream(s_up):
+                ev["up"][0].record(s_up)
+                for _ in range(reps):
+                    d_up.copy_(h_up, non_blocking=True)
+                ev["up"][1].record(s_up)
+        if dn:
+            with torch.cuda.stream(s_dn):
+                ev["dn"][0].record(s_dn)
+                for _ in range(reps):
+                    h_dn.copy_(d_dn, non_blocking=True)
+                ev["dn"][1].record(s_dn)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        out = {"wall_s": wall}
+        if up:
+            out["h2d_GB/s"] = reps * nbytes / (ev["up"][0].elapsed_time(ev["up"][1]) * 1e-3) / 1e9
+        if dn:
+            out["d2h_GB/s"] = reps * nbytes / (ev["dn"][0].elapsed_time(ev["dn"][1]) * 1e-3) / 1e9
+        if up and dn:
+            out["sum_GB/s_wall"] = 2 * reps * nbytes / wall / 1e9
+        return out
+
+    timed(True, True)                                     # warm-up
+    res = {"h2d_alone": timed(True, False), "d2h_alone": timed(False, True), "both": timed(True, True)}
+    import bsl6d_workloads as wl
+    npts = wl.CONFIGS[HEADLINE].npts
+    both = res["both"]
+    floor_ms = 8 * npts / (min(both["h2d_GB/s"], both["d2h_GB/s"]) * 1e9) * 1e3
+    print(json.dumps({"metric": "pinned host link, one cudaMemcpyAsync per direction per repetition", "unit": "GB/s",
+                      "bytes_per_copy": nbytes, "reps": reps, **res,
+                      "e2e_floor_ms_per_step_C5": floor_ms,
+                      "note": "floor = 8*npts bytes of C5 / the slower direction with both in flight: the step time of a "
+                              "perfectly overlapped stream of problems"}), flush=True)
+
+
 def run_paper_benchmark(args):
     """one 1-D interpolation per direction on 37^6 points, random alpha/dx in [-1,1] per
     point, odd stencil widths.  Reports, per width and direction, the time and GB/s in the paper's convention
@@ -981,6 +1055,9 @@ def run_paper_benchmark(args):
 
 def main():
     args = parse_args()
+    if args.link_benchmark:
+        run_link_benchmark(args)
+        return
     if args.paper_benchmark:
         run_paper_benchmark(args)
         return
