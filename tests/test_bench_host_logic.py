@@ -55,3 +55,16 @@ def test_reference_arm_other_ranks_exit_without_work():
     p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=120)
     assert p.returncode == 0 and p.stdout.strip() == ""
+
+
+def test_traffic_row_and_its_source_stamp():
+    """roofline.traffic comes from profiles/traffic.csv; the file's stamp (sha256 of the per-sweep kernels' source at
+    capture time) decides traffic_stale.  The stamp line must not be mistaken for a data row."""
+    import bench
+    val, src, stale = bench.read_traffic("C5")
+    assert val is not None and 5.7e10 < val < 5.9e10          # ~16 B/point x 48^3 x 32^3
+    assert "not measured in this run" in src
+    assert stale in (True, False)                             # a stamp is on record
+    assert len(bench.sweep_source_sha()) == 64
+    none, why, st = bench.read_traffic("no-such-workload")
+    assert none is None and st is None and "no ncu capture" in why
